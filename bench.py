@@ -1,0 +1,468 @@
+#!/usr/bin/env python
+"""bench.py — measures BASELINE.json's metric ("selective-scan fwd elements/s and achieved HBM
+GB/s (% of B200 peak) at 1 GPU") on the Mamba-scale config (configs[2], "cfg3": batch 8,
+d_inner 4096, N 16, L 2048, bf16 io, fp32 state) and prints ONE JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 1..5] [--L len] [--variant V] [--no-e2e] [--no-cpu-baseline]
+
+A "step" is one pass of the whole hot path (one selective_scan_fwd / affine_scan call) over
+one batch of seeded synthetic input.  For N > 1 (torchrun) every rank runs the same workload
+on its own batch (the path shards over independent rows with no collective: weak scaling),
+timing is the max over ranks, and `value` is all ranks' elements / that time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import torch  # noqa: E402
+
+from workloads import (config, make_affine_inputs, make_selective_inputs,  # noqa: E402
+                       to_f64_numpy)
+
+METRIC = "selective_scan_fwd_elements_per_s"
+L2_BYTES = 126 * (1 << 20)
+FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback ("of fallback")
+NOMINAL_HBM_GBS = 8000.0       # BASELINE.json north_star "~8 TB/s"
+SM_COUNT = 148
+MUFU_PER_CLK_PER_SM = 16       # ex2 results / clk / SM (4 per sub-partition), DESIGN.md §6
+FP32_PER_CLK_PER_SM = 128      # FP32 lane-ops / clk / SM
+
+
+# ----------------------------------------------------------------------------- helpers
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            mp = json.load(f)
+        return float(mp["hbm_gbs"]), "measured", mp
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback", {}
+
+
+def dtype_name(dt):
+    return {torch.float32: "f32", torch.bfloat16: "bf16"}[dt]
+
+
+def algorithmic_bytes(c, has_h0, has_D=True):
+    """SURVEY §8d.3 / DESIGN.md §5: the minimum bytes one call must move."""
+    sz = 2 if c.dtype == torch.bfloat16 else 4
+    if c.kind == "affine":
+        return c.num_seq * c.L * 3 * sz + 4 * c.num_seq * (1 + (1 if has_h0 else 0))
+    rows = c.batch * c.d_inner
+    return (3 * rows * c.L * sz + 2 * c.batch * c.N * c.L * sz + 4 * c.d_inner * c.N
+            + (4 * c.d_inner if has_D else 0) + 4 * rows * c.N * (1 + (1 if has_h0 else 0)))
+
+
+class ClockSampler:
+    """Samples SM clock / power / throttle reasons while the timed region runs (pynvml)."""
+    BITS = {0x1: "gpu_idle", 0x2: "applications_clocks_setting", 0x4: "sw_power_cap",
+            0x8: "hw_slowdown", 0x10: "sync_boost", 0x20: "sw_thermal_slowdown",
+            0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x100: "display_clock"}
+
+    def __init__(self, index, period=0.01):
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.power = [], set(), []
+        self._stop = threading.Event()
+        self._thread = None
+        self.max_mhz = None
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def _sample(self):
+        nv = self.nv
+        self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+        try:
+            self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+        except Exception:
+            pass
+        try:
+            mask = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+        except Exception:
+            mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        for bit, name in self.BITS.items():
+            if mask & bit and name != "gpu_idle":
+                self.reasons.add(name)
+
+    def _run(self):
+        while not self._stop.is_set():
+            try:
+                self._sample()
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.ok:
+            self._thread = threading.Thread(target=self._run, daemon=True)
+            self._thread.start()
+        return self
+
+    def __exit__(self, *exc):
+        if self._thread:
+            try:
+                self._sample()
+            except Exception:
+                pass
+            self._stop.set()
+            self._thread.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        s = sorted(self.samples)
+        out = {"sm_mhz": float(s[len(s) // 2]), "sm_max_mhz": float(self.max_mhz or 0),
+               "reasons": sorted(self.reasons), "samples": len(s)}
+        if self.power:
+            out["power_w_max"] = round(max(self.power), 1)
+        return out
+
+
+# ------------------------------------------------------------------------ the workload
+class Workload:
+    def __init__(self, args, device):
+        over = {}
+        if args.config == 5:
+            over["L"] = args.L or (1 << 16)
+        elif args.L:
+            over["L"] = args.L
+        self.c = config(args.config, **over)
+        self.device = device
+        self.kind = self.c.kind
+        self.sets = []
+
+    def build_sets(self, nsets, seed_offset=0):
+        import paper_2606_00601_b200 as lib
+        self.lib = lib
+        c = self.c
+        for i in range(nsets):
+            ci = config_with_seed(c, c.seed + 17 * i + seed_offset)
+            if self.kind == "affine":
+                inp = make_affine_inputs(ci, device=self.device)
+                out = {"h": torch.empty_like(inp["a"]),
+                       "h_last": torch.empty(c.num_seq, dtype=torch.float32, device=self.device)}
+            else:
+                inp = make_selective_inputs(ci, device=self.device)
+                out = {"y": torch.empty_like(inp["x"]),
+                       "h_last": torch.empty((c.batch, c.d_inner, c.N), dtype=torch.float32,
+                                             device=self.device)}
+            self.sets.append((inp, out))
+        self.has_h0 = self.sets[0][0].get("h0") is not None
+        self.bytes = algorithmic_bytes(c, self.has_h0)
+
+    def launch(self, i, variant=0):
+        inp, out = self.sets[i % len(self.sets)]
+        if self.kind == "affine":
+            self.lib.affine_scan_ex(inp["a"], inp["u"], inp["h0"], out["h"], out["h_last"], variant)
+        else:
+            self.lib.selective_scan_fwd_ex(inp["x"], inp["delta"], inp["A"], inp["B"], inp["C"],
+                                           inp["D"], inp["h0"], out["y"], out["h_last"], variant)
+
+    # end-to-end through the C-ABI with HOST buffers (pinned)
+    def build_host(self):
+        inp, out = self.sets[0]
+        self.h_in = {k: (None if v is None else v.cpu().pin_memory()) for k, v in inp.items()}
+        self.h_out = {k: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k, v in out.items()}
+        self.h2d = sum(v.numel() * v.element_size() for v in self.h_in.values() if v is not None)
+        self.d2h = sum(v.numel() * v.element_size() for v in self.h_out.values())
+
+    def launch_host(self):
+        i, o = self.h_in, self.h_out
+        if self.kind == "affine":
+            self.lib.affine_scan_host(i["a"], i["u"], i["h0"], o["h"], o["h_last"])
+        else:
+            self.lib.selective_scan_fwd_host(i["x"], i["delta"], i["A"], i["B"], i["C"], i["D"],
+                                             i["h0"], o["y"], o["h_last"])
+
+    def describe(self, world):
+        c = self.c
+        d = {"workload": c.name, "call": "affine_scan" if self.kind == "affine"
+             else "selective_scan_fwd", "seed": c.seed}
+        if self.kind == "affine":
+            d.update(num_seq=c.num_seq, L=c.L)
+        else:
+            d.update(batch=c.batch, d_inner=c.d_inner, N=c.N, L=c.L)
+        d["io_dtype"] = dtype_name(c.dtype)
+        d["parallelism"] = f"independent_batches_x{world}" if world > 1 else "single_gpu"
+        return d
+
+
+def config_with_seed(c, seed):
+    from dataclasses import replace
+    return replace(c, seed=seed)
+
+
+# ----------------------------------------------------------------- CPU baseline (oracle)
+def oracle_sample_runner(c, device_inputs, seed=0):
+    """Returns (run(n_units) -> elements processed, unit name, max units).  The sample is the
+    first n rows / sequences of the SAME workload; the oracle runs as it stands (1 thread)."""
+    import oracle
+    inp = device_inputs
+    if c.kind == "affine":
+        a, u = inp["a"], inp["u"]
+        h0 = inp["h0"]
+
+        def run(n):
+            n = max(1, min(n, c.num_seq))
+            oracle.affine_scan(to_f64_numpy(a[:n]), to_f64_numpy(u[:n]),
+                               None if h0 is None else to_f64_numpy(h0[:n]))
+            return n * c.L
+        return run, "sequences", c.num_seq
+
+    host = {k: (None if v is None else to_f64_numpy(v[:1] if k in ("x", "delta", "B", "C", "h0")
+                                                    else v)) for k, v in inp.items()}
+
+    def run(n):
+        n = max(1, min(n, c.d_inner))
+        oracle.selective_scan_fwd(host["x"][:, :n], host["delta"][:, :n], host["A"][:n],
+                                  host["B"], host["C"], host["D"][:n],
+                                  None if host["h0"] is None else host["h0"][:, :n])
+        return n * c.L
+    return run, "rows_of_batch0", c.d_inner
+
+
+def time_oracle(c, inputs, target_s):
+    run, unit, max_units = oracle_sample_runner(c, inputs)
+    probe = max(1, min(max_units, 8))
+    run(1)                                   # load/compile the C oracle outside the timing
+    t0 = time.perf_counter()
+    el = run(probe)
+    dt = max(time.perf_counter() - t0, 1e-6)
+    n = int(max(1, min(max_units, probe * target_s / dt)))
+    t0 = time.perf_counter()
+    el = run(n)
+    dt = time.perf_counter() - t0
+    return {"value": el / dt, "unit": "elements/s", "cores": 1, "kind": "oracle",
+            "sample": f"first {n} {unit} of the workload ({el} elements, {dt:.2f} s, float64, "
+                      f"1 thread)"}
+
+
+# ------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    rank, world, _ = dist_env()
+    if rank != 0:
+        return 0
+    w = Workload(args, "cpu")
+    c = w.c
+    inputs = (make_affine_inputs if c.kind == "affine" else make_selective_inputs)(
+        c if c.elements <= (1 << 24) else shrink_for_cpu(c), device="cpu")
+    run, unit, max_units = oracle_sample_runner(c if c.elements <= (1 << 24) else shrink_for_cpu(c),
+                                                inputs)
+    # size the per-step sample so that (steps + warmup) steps end within ~2 minutes
+    run(1)
+    t0 = time.perf_counter()
+    el = run(4)
+    per_unit = (time.perf_counter() - t0) / 4
+    budget = 120.0 / max(1, args.steps + args.warmup)
+    n = int(max(1, min(max_units, budget / max(per_unit, 1e-9))))
+    for _ in range(args.warmup):
+        run(n)
+    t0 = time.perf_counter()
+    elements = 0
+    for _ in range(args.steps):
+        elements += run(n)
+    dt = time.perf_counter() - t0
+    value = elements / dt
+    sample = f"{n} {unit} per step ({elements // max(1, args.steps)} elements/step), float64, 1 thread"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": "elements/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, workloads/gen.py)",
+        "config": w.describe(1),
+        "cpu_baseline": {"value": value, "unit": "elements/s", "cores": 1, "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": "elements/s", "h2d_bytes_per_step": 0,
+                "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+def shrink_for_cpu(c):
+    """Host-side stand-in for the big configs: same distributions and L, fewer rows, so the
+    reference arm never materialises hundreds of MB it will not scan."""
+    from dataclasses import replace
+    if c.kind == "affine":
+        return replace(c, num_seq=min(c.num_seq, max(1, (1 << 22) // c.L)))
+    return replace(c, batch=1, d_inner=min(c.d_inner, 512))
+
+
+# ------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py (impl ours) needs a CUDA device; there is no CPU fallback")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    from paper_2606_00601_b200.sharding import max_over_ranks
+
+    import paper_2606_00601_b200 as lib
+    w = Workload(args, device)
+    c = w.c
+    step_bytes = algorithmic_bytes(c, c.kind == "affine" and c.h0_recipe == "normal")
+    nsets = max(2, -(-4 * L2_BYTES // step_bytes)) if step_bytes < 4 * L2_BYTES else 2
+    nsets = min(nsets, 64)
+    w.build_sets(nsets, seed_offset=1000 * rank)
+    variant = args.variant
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- warm-up
+    for i in range(max(args.warmup, 3)):
+        w.launch(i, variant)
+    torch.cuda.synchronize()
+    chosen = lib.last_variant()
+
+    # ---- timed region: K steps, device time (CUDA events on the launching stream)
+    K = args.steps
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(K)]
+    t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    launches0 = lib.launch_count()
+    barrier()
+    with ClockSampler(local) as clocks:
+        t_begin.record()
+        for i in range(K):
+            ev[i][0].record()
+            w.launch(i, variant)
+            ev[i][1].record()
+        t_end.record()
+        torch.cuda.synchronize()
+    barrier()
+    launches = lib.launch_count() - launches0
+    total_ms = max_over_ranks(t_begin.elapsed_time(t_end), device)
+    per_launch_ms = sorted(a.elapsed_time(b) for a, b in ev)
+    kernel_ms = sum(per_launch_ms) / K
+    ms_per_step = total_ms / K
+    elements = c.elements * world
+    value = elements / (ms_per_step * 1e-3)
+
+    peak, peak_kind, mp = measured_peaks()
+    achieved = w.bytes / (kernel_ms * 1e-3) / 1e9
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
+            traffic = json.load(f).get(c.name)
+    except Exception:
+        pass
+    clk = clocks.summary()
+    roofline = {"bound": "hbm", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                "frac": round(achieved / peak, 4), "traffic": traffic, "peak_kind": peak_kind,
+                "algorithmic_bytes": w.bytes, "kernel_ms": round(kernel_ms, 5),
+                "kernel_ms_min": round(per_launch_ms[0], 5),
+                "kernel_ms_median": round(per_launch_ms[K // 2], 5),
+                "frac_of_nominal_8TBps": round(achieved / NOMINAL_HBM_GBS, 4),
+                "kernel": lib.VARIANT_NAMES.get(chosen, str(chosen))}
+    line = {
+        "metric": METRIC, "value": value, "unit": "elements/s", "n_gpus": world, "steps": K,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic (seeded, workloads/gen.py; BASELINE.json distributions)",
+        "config": {**w.describe(world),
+                   "l2": f"{nsets} rotating input/output sets x {step_bytes / 1e6:.1f} MB "
+                         f"(> 126 MB L2 between reuses)"},
+        "clocks": clk, "gpu_launches": launches, "roofline": roofline,
+        "hbm_gbs_achieved": round(achieved, 1),
+    }
+    if c.kind == "selective":
+        # the binding roofline of this path: exp on the SFU and FP32 lane-ops
+        mhz = clk.get("sm_mhz") or clk.get("sm_max_mhz") or 1965.0
+        steps_state = c.elements * c.N
+        mufu_ms = steps_state / (MUFU_PER_CLK_PER_SM * SM_COUNT * mhz * 1e6) * 1e3
+        fp32_ms = 4 * steps_state / (FP32_PER_CLK_PER_SM * SM_COUNT * mhz * 1e6) * 1e3
+        line["roofline_alu"] = {
+            "bound": "alu", "unit": "state-steps/s",
+            "achieved": steps_state / (kernel_ms * 1e-3),
+            "peak": steps_state / (mufu_ms * 1e-3),
+            "frac": round(mufu_ms / kernel_ms, 4),
+            "note": "peak = 16 MUFU.EX2/clk/SM x 148 SMs x sampled SM clock, 1 exp per "
+                    "state-step; fp32_wall_ms is 4 FP32 lane-ops per state-step at 128/clk/SM",
+            "mufu_wall_ms": round(mufu_ms, 4), "fp32_wall_ms": round(fp32_ms, 4),
+            "sm_mhz_used": mhz}
+
+    # ---- end to end through the C-ABI with host buffers
+    if not args.no_e2e:
+        w.build_host()
+        for _ in range(2):
+            w.launch_host()
+        barrier()
+        ke = max(3, min(args.e2e_steps, K))
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            w.launch_host()          # synchronises the stream before returning
+        torch.cuda.synchronize()
+        e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / ke, device)
+        line["e2e"] = {"value": elements / (e2e_ms * 1e-3), "unit": "elements/s",
+                       "h2d_bytes_per_step": w.h2d, "d2h_bytes_per_step": w.d2h,
+                       "steps": ke, "ms_per_step": e2e_ms,
+                       "api": f"{'affine_scan' if c.kind == 'affine' else 'selective_scan_fwd'}"
+                              "_host (pinned host buffers, H2D + kernel + D2H per step)"}
+
+    # ---- the oracle timed beside it (rank 0, N=1 only)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = time_oracle(c, w.sets[0][0], args.cpu_seconds)
+
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3)")
+    ap.add_argument("--L", type=int, default=0, help="sequence length override (config 5 sweep)")
+    ap.add_argument("--variant", type=int, default=0, help="force an affinescan_variant")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=10)
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    if args.steps < 1:
+        ap.error("--steps must be >= 1")
+    sys.exit(run_reference(args) if args.impl == "reference" else run_ours(args))
+
+
+if __name__ == "__main__":
+    main()

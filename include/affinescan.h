@@ -1,0 +1,180 @@
+/*
+ * affinescan.h — C ABI of libaffinescan: the affine-pair associative scan of
+ * arxiv/paper_2606_00601 ("ScanWeaver") and its main instance, the Mamba-style
+ * fused selective-scan forward, as hand-written CUDA kernels for sm_100a (B200).
+ *
+ * Citations:  P:<n>  = line n of /root/reference/PAPER.md
+ *             BJ     = BASELINE.json north_star / configs
+ *             Q<k>   = reading k in DESIGN.md ("Readings of the paper")
+ *
+ * Conventions common to every entry point
+ *   - Plain pointers and sizes only.  Unless the name ends in `_host`, every data
+ *     pointer is a DEVICE pointer on the current CUDA device; `_host` entry points
+ *     take HOST pointers (pinned or pageable) and do the copies themselves.
+ *   - All tensors are dense, row-major, last index contiguous; no strides.
+ *   - The caller owns every buffer.  Inputs are never written.  Outputs must not
+ *     alias inputs (in-place is unsupported).
+ *   - Device entry points are asynchronous on `cuda_stream` (a cudaStream_t cast to
+ *     void*; NULL = the legacy default stream): they enqueue work and return without
+ *     synchronising.  `_host` entry points synchronise `cuda_stream` before returning.
+ *   - The library owns only a small per-(device, stream) scratch for the decoupled
+ *     look-back tile descriptors, grown on demand and freed at unload.
+ *   - Errors are integer status codes (affinescan_status); nothing aborts, throws or
+ *     prints.  Misaligned pointers or an L that is not a multiple of the 128-bit
+ *     vector width are NOT errors: a scalar-load kernel is chosen.
+ *   - State and accumulation are fp32; io dtype is fp32 or bf16; outputs are rounded
+ *     to the io dtype with round-to-nearest-even; h_last is always fp32.
+ *   - Results are bitwise reproducible run to run for a given variant (values are
+ *     never accumulated with atomics).
+ */
+#ifndef AFFINESCAN_H_
+#define AFFINESCAN_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(_WIN32)
+#define AFFINESCAN_API
+#else
+#define AFFINESCAN_API __attribute__((visibility("default")))
+#endif
+
+typedef enum affinescan_status {
+    AFFINESCAN_OK = 0,
+    AFFINESCAN_ERR_NULL = 1,        /* a required pointer is NULL                         */
+    AFFINESCAN_ERR_SHAPE = 2,       /* negative size, or a size product overflows int64   */
+    AFFINESCAN_ERR_DTYPE = 3,       /* io_dtype is not an affinescan_dtype                */
+    AFFINESCAN_ERR_UNSUPPORTED = 4, /* N outside [1, AFFINESCAN_MAX_N]; unknown variant;
+                                       a forced variant that cannot run this shape        */
+    AFFINESCAN_ERR_CUDA = 5         /* a CUDA runtime call failed; see
+                                       affinescan_last_cuda_error()                       */
+} affinescan_status;
+
+typedef enum affinescan_dtype {
+    AFFINESCAN_F32 = 0,  /* IEEE binary32 */
+    AFFINESCAN_BF16 = 1  /* bfloat16      */
+} affinescan_dtype;
+
+#define AFFINESCAN_MAX_N 64
+
+/* Kernel variants.  AUTO picks from the shape; the others force one schedule (tests,
+ * ablations, benchmarks). */
+typedef enum affinescan_variant {
+    AFFINESCAN_VARIANT_AUTO = 0,
+    /* affine_scan */
+    AFFINESCAN_AFFINE_LOOKBACK = 1, /* single pass over the flattened [num_seq*L] stream;
+                                       decoupled look-back carry between tiles; sequence
+                                       heads are reset pairs (0, a0*h0+u0)  (BJ)          */
+    AFFINESCAN_AFFINE_CTA_LOOP = 2, /* one CTA per sequence, loop over L with the carry in
+                                       a register (BJ "carry ... in a CTA loop")          */
+    AFFINESCAN_AFFINE_BLELLOCH = 3, /* ABLATION: the paper's shared-memory Blelloch
+                                       upsweep / root init / downsweep / reconstruction
+                                       (P:103-107), CTA-loop carry             */
+    /* selective_scan_fwd */
+    AFFINESCAN_SELECTIVE_WARP_ROW = 11, /* one warp per (b,d) row, lanes own consecutive
+                                           chunks of L, warp-shuffle pair scan            */
+    AFFINESCAN_SELECTIVE_LANE_ROW = 12  /* one lane per (b,d) row, sequential in L, x/Δ/y
+                                           and B/C tiles staged in shared memory by TMA
+                                           bulk copies (needs d_inner % 32 == 0)          */
+} affinescan_variant;
+
+/* ------------------------------------------------------------------------------------
+ * affine_scan — inclusive scan of the affine recurrence
+ *
+ *     h[s,t] = a[s,t] * h[s,t-1] + u[s,t],   h[s,-1] = h0[s],   t = 0..L-1
+ *     h_last[s] = h[s,L-1]                   (= h0[s] when L == 0)
+ *
+ * i.e. the prefix scan over the pairs (A_t,U_t) = (a_t, b_t x_t) (Eq.6) under
+ * (A2,U2)(+)(A1,U1) = (A2 A1, A2 U1 + U2) (Eq.7), which reproduces the
+ * sequential recurrence h_t = a_t h_{t-1} + b_t x_t (Eq.1, Eq.3) with the
+ * initial state h_0 of P:81 Eq.5.  Also covers the weighted-prefix recurrence
+ * h_t = alpha_t h_{t-1} + beta_t (Eq.10) with a = alpha, u = beta.
+ *
+ *   a, u     [num_seq, L]  io dtype   in
+ *   h0       [num_seq]     fp32       in, NULL => 0
+ *   h        [num_seq, L]  io dtype   out
+ *   h_last   [num_seq]     fp32       out, NULL => not written
+ *
+ * num_seq == 0 or L == 0 is OK (h_last <- h0 or 0).  Returns an affinescan_status.
+ * ------------------------------------------------------------------------------------ */
+AFFINESCAN_API int affine_scan(const void* a, const void* u, const float* h0, void* h,
+                               float* h_last, int64_t num_seq, int64_t L, int io_dtype,
+                               void* cuda_stream);
+
+/* Same, forcing a kernel variant (AFFINESCAN_VARIANT_AUTO or an AFFINESCAN_AFFINE_*). */
+AFFINESCAN_API int affine_scan_ex(const void* a, const void* u, const float* h0, void* h,
+                                  float* h_last, int64_t num_seq, int64_t L, int io_dtype,
+                                  int variant, void* cuda_stream);
+
+/* Same computation with HOST buffers: copies a, u, h0 to the device, runs the kernel,
+ * copies h and h_last back, and synchronises `cuda_stream`.  Device staging buffers are
+ * owned and cached by the library. */
+AFFINESCAN_API int affine_scan_host(const void* a, const void* u, const float* h0, void* h,
+                                    float* h_last, int64_t num_seq, int64_t L, int io_dtype,
+                                    void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
+ * selective_scan_fwd — Mamba-style fused forward selective scan (BJ north_star):
+ *
+ *     a_t[d,n] = exp(delta_t[d] * A[d,n])              discretisation (BJ)
+ *     u_t[d,n] = delta_t[d] * B_t[n] * x_t[d]          b_t = delta_t B_t (BJ); U = b x
+ *     h_t[d,n] = a_t[d,n] * h_{t-1}[d,n] + u_t[d,n]    (Eq.3), h_{-1} = h0
+ *     y_t[d]   = sum_n C_t[n] * h_t[d,n] + D[d] * x_t[d]   (BJ; Eq.4 is N=1, D=0)
+ *
+ * h is never written to memory; only y and the final state are.
+ *
+ *   x, delta [batch, d_inner, L]  io dtype  in   (delta > 0: softplus already applied)
+ *   A        [d_inner, N]         fp32      in   (negative => a in (0,1))
+ *   B, C     [batch, N, L]        io dtype  in
+ *   D        [d_inner]            fp32      in, NULL => no skip term
+ *   h0       [batch, d_inner, N]  fp32      in, NULL => 0
+ *   y        [batch, d_inner, L]  io dtype  out
+ *   h_last   [batch, d_inner, N]  fp32      out, NULL => not written
+ *
+ * 1 <= N <= AFFINESCAN_MAX_N (N = 16 is the tuned case).  exp is evaluated as
+ * ex2.approx.ftz.f32(delta * (A * log2 e)) (Q11).  batch, d_inner or L == 0 is OK.
+ * ------------------------------------------------------------------------------------ */
+AFFINESCAN_API int selective_scan_fwd(const void* x, const void* delta, const float* A,
+                                      const void* B, const void* C, const float* D,
+                                      const float* h0, void* y, float* h_last, int batch,
+                                      int d_inner, int N, int64_t L, int io_dtype,
+                                      void* cuda_stream);
+
+/* Same, forcing a kernel variant (AUTO or an AFFINESCAN_SELECTIVE_*). */
+AFFINESCAN_API int selective_scan_fwd_ex(const void* x, const void* delta, const float* A,
+                                         const void* B, const void* C, const float* D,
+                                         const float* h0, void* y, float* h_last, int batch,
+                                         int d_inner, int N, int64_t L, int io_dtype,
+                                         int variant, void* cuda_stream);
+
+/* Same computation with HOST buffers (see affine_scan_host). */
+AFFINESCAN_API int selective_scan_fwd_host(const void* x, const void* delta, const float* A,
+                                           const void* B, const void* C, const float* D,
+                                           const float* h0, void* y, float* h_last,
+                                           int batch, int d_inner, int N, int64_t L,
+                                           int io_dtype, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
+ * Introspection (no device work)
+ * ------------------------------------------------------------------------------------ */
+/* Static, NUL-terminated description of a status code. */
+AFFINESCAN_API const char* affinescan_status_string(int status);
+/* cudaError_t of the last AFFINESCAN_ERR_CUDA on the calling thread (0 if none). */
+AFFINESCAN_API int affinescan_last_cuda_error(void);
+/* affinescan_variant the last successful call on the calling thread ran (0 if none or
+ * if the call was a no-op on an empty shape). */
+AFFINESCAN_API int affinescan_last_variant(void);
+/* Number of kernel launches this process has issued through the library so far. */
+AFFINESCAN_API int64_t affinescan_launch_count(void);
+/* Library version: major*10000 + minor*100 + patch. */
+AFFINESCAN_API int affinescan_version(void);
+/* Frees the cached scratch / staging buffers of the current device (synchronises it). */
+AFFINESCAN_API int affinescan_release_cache(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFFINESCAN_H_ */

@@ -1,0 +1,238 @@
+"""ctypes binding of libaffinescan (include/affinescan.h) — argument marshalling only.
+
+Every function has the name and argument order of its C entry point.  Tensors are
+torch tensors (PyTorch is used for device memory and streams only); every step of
+the computation runs in the library's CUDA kernels.  There is NO fallback: if the
+shared library is missing or a call fails, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+import torch
+
+from . import build as _build
+
+F32 = 0
+BF16 = 1
+
+VARIANT_AUTO = 0
+AFFINE_LOOKBACK = 1
+AFFINE_CTA_LOOP = 2
+AFFINE_BLELLOCH = 3
+SELECTIVE_WARP_ROW = 11
+SELECTIVE_LANE_ROW = 12
+
+VARIANT_NAMES = {
+    0: "auto", 1: "affine_lookback", 2: "affine_cta_loop", 3: "affine_blelloch",
+    11: "selective_warp_row", 12: "selective_lane_row",
+}
+
+_vp = ctypes.c_void_p
+_i64 = ctypes.c_int64
+_int = ctypes.c_int
+
+_SIGNATURES = {
+    "affine_scan": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _vp]),
+    "affine_scan_ex": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _int, _vp]),
+    "affine_scan_host": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _vp]),
+    "selective_scan_fwd": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _vp]),
+    "selective_scan_fwd_ex": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _int, _vp]),
+    "selective_scan_fwd_host": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _vp]),
+    "affinescan_status_string": (ctypes.c_char_p, [_int]),
+    "affinescan_last_cuda_error": (_int, []),
+    "affinescan_last_variant": (_int, []),
+    "affinescan_launch_count": (_i64, []),
+    "affinescan_version": (_int, []),
+    "affinescan_release_cache": (_int, []),
+}
+
+
+class AffineScanError(RuntimeError):
+    def __init__(self, fn: str, status: int, detail: str, cuda_error: int):
+        self.status = status
+        self.cuda_error = cuda_error
+        extra = f" (cudaError {cuda_error})" if status == 5 else ""
+        super().__init__(f"{fn} failed: status {status}: {detail}{extra}")
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _build.LIB_PATH
+
+
+def declared_symbols(header_path: str | None = None):
+    """Names of every AFFINESCAN_API function declared in include/affinescan.h."""
+    if header_path is None:
+        header_path = os.path.join(_build.ROOT, "include", "affinescan.h")
+    with open(header_path) as f:
+        text = f.read()
+    return re.findall(r"AFFINESCAN_API\s+[\w\s\*]+?\b(\w+)\s*\(", text)
+
+
+def load():
+    """dlopen libaffinescan.so (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is None:
+        path = library_path()
+        if not os.path.exists(path):
+            raise FileNotFoundError(
+                f"{path} not found: build it with `python -m paper_2606_00601_b200.build` "
+                "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = ctypes.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(lib, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = lib
+    return _lib
+
+
+def _check(fn: str, status: int):
+    if status != 0:
+        lib = load()
+        raise AffineScanError(fn, status, lib.affinescan_status_string(status).decode(),
+                              lib.affinescan_last_cuda_error())
+
+
+def _io_dtype(t: torch.Tensor) -> int:
+    if t.dtype == torch.float32:
+        return F32
+    if t.dtype == torch.bfloat16:
+        return BF16
+    raise TypeError(f"io dtype must be float32 or bfloat16, got {t.dtype}")
+
+
+def _ptr(t, *, dtype=None, shape=None, device=None, name="tensor"):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor):
+        raise TypeError(f"{name}: expected a torch.Tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name}: expected {dtype}, got {t.dtype}")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"{name}: expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name}: must be contiguous (dense row-major)")
+    if device is not None and t.device.type != device:
+        raise ValueError(f"{name}: expected a {device} tensor, got {t.device}")
+    return t.data_ptr() if t.numel() else (t.data_ptr() or None)
+
+
+def _stream_ptr(stream, ref: torch.Tensor):
+    if stream is None:
+        if ref.is_cuda:
+            return torch.cuda.current_stream(ref.device).cuda_stream
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream
+    return int(stream)
+
+
+# ------------------------------------------------------------------------ affine_scan
+def _affine_args(a, u, h0, h, h_last, device):
+    if a.dim() != 2:
+        raise ValueError("a must be [num_seq, L]")
+    S, L = a.shape
+    io = _io_dtype(a)
+    return (
+        _ptr(a, shape=(S, L), device=device, name="a"),
+        _ptr(u, dtype=a.dtype, shape=(S, L), device=device, name="u"),
+        _ptr(h0, dtype=torch.float32, shape=(S,), device=device, name="h0"),
+        _ptr(h, dtype=a.dtype, shape=(S, L), device=device, name="h"),
+        _ptr(h_last, dtype=torch.float32, shape=(S,), device=device, name="h_last"),
+        S, L, io,
+    )
+
+
+def affine_scan(a, u, h0, h, h_last, stream=None):
+    """h[s,t] = a[s,t]*h[s,t-1] + u[s,t]; device tensors; async on ``stream``."""
+    args = _affine_args(a, u, h0, h, h_last, "cuda")
+    with torch.cuda.device(a.device):
+        _check("affine_scan", load().affine_scan(*args, _stream_ptr(stream, a)))
+
+
+def affine_scan_ex(a, u, h0, h, h_last, variant, stream=None):
+    args = _affine_args(a, u, h0, h, h_last, "cuda")
+    with torch.cuda.device(a.device):
+        _check("affine_scan_ex", load().affine_scan_ex(*args, int(variant), _stream_ptr(stream, a)))
+
+
+def affine_scan_host(a, u, h0, h, h_last, stream=None):
+    """Same with HOST tensors (pinned or pageable); synchronises before returning."""
+    args = _affine_args(a, u, h0, h, h_last, "cpu")
+    _check("affine_scan_host", load().affine_scan_host(*args, _stream_ptr(stream, a)))
+
+
+# ----------------------------------------------------------------- selective_scan_fwd
+def _selective_args(x, delta, A, B, C, D, h0, y, h_last, device):
+    if x.dim() != 3:
+        raise ValueError("x must be [batch, d_inner, L]")
+    if A.dim() != 2:
+        raise ValueError("A must be [d_inner, N]")
+    batch, d_inner, L = x.shape
+    N = A.shape[1]
+    io = _io_dtype(x)
+    f32 = torch.float32
+    return (
+        _ptr(x, shape=(batch, d_inner, L), device=device, name="x"),
+        _ptr(delta, dtype=x.dtype, shape=(batch, d_inner, L), device=device, name="delta"),
+        _ptr(A, dtype=f32, shape=(d_inner, N), device=device, name="A"),
+        _ptr(B, dtype=x.dtype, shape=(batch, N, L), device=device, name="B"),
+        _ptr(C, dtype=x.dtype, shape=(batch, N, L), device=device, name="C"),
+        _ptr(D, dtype=f32, shape=(d_inner,), device=device, name="D"),
+        _ptr(h0, dtype=f32, shape=(batch, d_inner, N), device=device, name="h0"),
+        _ptr(y, dtype=x.dtype, shape=(batch, d_inner, L), device=device, name="y"),
+        _ptr(h_last, dtype=f32, shape=(batch, d_inner, N), device=device, name="h_last"),
+        batch, d_inner, N, L, io,
+    )
+
+
+def selective_scan_fwd(x, delta, A, B, C, D, h0, y, h_last, stream=None):
+    """Fused Mamba-style forward selective scan; device tensors; async on ``stream``."""
+    args = _selective_args(x, delta, A, B, C, D, h0, y, h_last, "cuda")
+    with torch.cuda.device(x.device):
+        _check("selective_scan_fwd", load().selective_scan_fwd(*args, _stream_ptr(stream, x)))
+
+
+def selective_scan_fwd_ex(x, delta, A, B, C, D, h0, y, h_last, variant, stream=None):
+    args = _selective_args(x, delta, A, B, C, D, h0, y, h_last, "cuda")
+    with torch.cuda.device(x.device):
+        _check("selective_scan_fwd_ex",
+               load().selective_scan_fwd_ex(*args, int(variant), _stream_ptr(stream, x)))
+
+
+def selective_scan_fwd_host(x, delta, A, B, C, D, h0, y, h_last, stream=None):
+    """Same with HOST tensors (pinned or pageable); synchronises before returning."""
+    args = _selective_args(x, delta, A, B, C, D, h0, y, h_last, "cpu")
+    _check("selective_scan_fwd_host",
+           load().selective_scan_fwd_host(*args, _stream_ptr(stream, x)))
+
+
+# ------------------------------------------------------------------------ introspection
+def status_string(status: int) -> str:
+    return load().affinescan_status_string(int(status)).decode()
+
+
+def last_cuda_error() -> int:
+    return load().affinescan_last_cuda_error()
+
+
+def last_variant() -> int:
+    return load().affinescan_last_variant()
+
+
+def launch_count() -> int:
+    return load().affinescan_launch_count()
+
+
+def version() -> int:
+    return load().affinescan_version()
+
+
+def release_cache() -> None:
+    _check("affinescan_release_cache", load().affinescan_release_cache())

@@ -1,0 +1,394 @@
+// affine_scan.cuh — kernels for affine_scan (include/affinescan.h):
+//   h[s,t] = a[s,t]*h[s,t-1] + u[s,t]   as a prefix scan over pairs (a_t,u_t) under
+//   (A2,U2)(+)(A1,U1) = (A2*A1, A2*U1+U2)           (Eq.6, Eq.7)
+//
+// Schedule (BJ north_star; SURVEY §8a A1,A4-A8,A11): coalesced 128-bit loads; every
+// thread composes its VEC consecutive steps in registers; pairs are combined across
+// the warp with __shfl_up_sync and across warps through shared memory; the carry
+// crosses tiles either by decoupled look-back over a flattened [num_seq*L] stream
+// (sequence heads become reset pairs (0, a0*h0+u0), a left zero of (+)) or in a
+// CTA loop with the carry in a register.  The paper's Blelloch up/down-sweep
+// is kept as a shared-memory ablation only.
+#pragma once
+
+#include "common.cuh"
+
+namespace affinescan {
+
+// ------------------------------------------------------------------ tile descriptors
+// One descriptor per tile = two 64-bit words {status:32 | float bits:32}: word 0 carries
+// P, word 1 carries U.  Each word is written with ONE 64-bit store, so a reader that
+// sees equal non-empty statuses in both words holds a consistent pair.  INCLUSIVE
+// descriptors carry (0, h_end): the state after the tile, as a left-zero pair.
+constexpr unsigned kDescEmpty = 0u;
+constexpr unsigned kDescAggregate = 1u;
+constexpr unsigned kDescInclusive = 2u;
+
+__device__ __forceinline__ void desc_store(unsigned long long* d, unsigned status, Pair v)
+{
+    const unsigned long long hi = static_cast<unsigned long long>(status) << 32;
+    const unsigned long long w0 = hi | __float_as_uint(v.P);
+    const unsigned long long w1 = hi | __float_as_uint(v.U);
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(d), "l"(w0) : "memory");
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(d + 1), "l"(w1) : "memory");
+}
+
+__device__ __forceinline__ unsigned desc_load(const unsigned long long* d, Pair& v)
+{
+    unsigned long long w0, w1;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w0) : "l"(d) : "memory");
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w1) : "l"(d + 1) : "memory");
+    const unsigned s0 = static_cast<unsigned>(w0 >> 32);
+    const unsigned s1 = static_cast<unsigned>(w1 >> 32);
+    v.P = __uint_as_float(static_cast<unsigned>(w0));
+    v.U = __uint_as_float(static_cast<unsigned>(w1));
+    return s0 == s1 ? s0 : kDescEmpty;  // torn read (mid-transition) => retry
+}
+
+// ------------------------------------------------------------------ per-thread tile state
+// A CTA tile is WARPS*32*VEC*J elements.  Warp w owns a contiguous 32*VEC*J slice; inside
+// it, lane l's j-th vector starts at j*32*VEC + l*VEC, so every 128-bit access of a warp
+// is one fully coalesced 512-byte request.
+template <int VEC, int J>
+struct TileRegs {
+    float av[J][VEC];
+    float uv[J][VEC];
+    Pair excl[J];  // composition of lanes < lane within vector-row j
+    Pair tot[J];   // composition of all 32 lanes of vector-row j
+};
+
+// Thread-local compose + warp combine (A5) of one vector-row.
+template <int VEC, int J>
+__device__ __forceinline__ void row_scan(TileRegs<VEC, J>& r, int j, int lane)
+{
+    Pair loc{r.av[j][0], r.uv[j][0]};
+#pragma unroll
+    for (int k = 1; k < VEC; ++k) loc = compose(Pair{r.av[j][k], r.uv[j][k]}, loc);
+    const Pair inc = warp_inclusive_scan(loc, lane);
+    Pair ex = shfl_up_pair(inc, 1);
+    if (lane == 0) ex = identity_pair();
+    r.excl[j] = ex;
+    r.tot[j] = shfl_pair(inc, 31);
+}
+
+template <int VEC, int J>
+__device__ __forceinline__ Pair warp_total(const TileRegs<VEC, J>& r)
+{
+    Pair w = r.tot[0];
+#pragma unroll
+    for (int j = 1; j < J; ++j) w = compose(r.tot[j], w);
+    return w;
+}
+
+// Position of flat element index base+off inside its sequence: (s, t).  q0 = base / L and
+// r0 = base % L are computed once per tile; off < tile size < 2^31.
+__device__ __forceinline__ void seq_pos(long long q0, long long r0, int off, long long L,
+                                        int tile_elems, long long& s, long long& t)
+{
+    t = r0 + off;
+    s = q0;
+    if (t >= L) {
+        if (L >= tile_elems) {  // at most one sequence boundary inside the tile
+            t -= L;
+            s += 1;
+        } else {  // t < L + tile_elems < 2^32
+            const unsigned q = static_cast<unsigned>(t) / static_cast<unsigned>(L);
+            t -= static_cast<long long>(q) * L;
+            s += q;
+        }
+    }
+}
+
+// ====================================================================================
+// Variant AFFINESCAN_AFFINE_LOOKBACK: single pass, decoupled look-back
+// ====================================================================================
+template <typename T, int VEC, int J, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
+                            const float* __restrict__ h0, T* __restrict__ h,
+                            float* __restrict__ h_last, long long total, long long L,
+                            unsigned long long* __restrict__ desc, unsigned* __restrict__ ticket)
+{
+    constexpr int kWarpElems = 32 * VEC * J;
+    constexpr int kTile = WARPS * kWarpElems;
+    using Acc = Access<T, VEC, true>;
+
+    __shared__ unsigned s_tile;
+    __shared__ long long s_q0, s_r0;
+    __shared__ Pair s_warp[WARPS];
+    __shared__ float s_hin;
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+
+    // Tile ids come from a ticket so that every predecessor tile is already running
+    // when its successor looks back (forward progress without relying on block order).
+    if (threadIdx.x == 0) {
+        const unsigned tk = atomicAdd(ticket, 1u);
+        const long long b = static_cast<long long>(tk) * kTile;
+        s_tile = tk;
+        s_q0 = b / L;
+        s_r0 = b % L;
+    }
+    __syncthreads();
+    const unsigned tile = s_tile;
+    const long long base = static_cast<long long>(tile) * kTile;
+    const long long q0 = s_q0, r0 = s_r0;
+
+    TileRegs<VEC, J> r;
+    // ---- A1: loads (all J vectors issued before first use)
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+        if (base + off < total) {
+            Acc::load(a + base + off, r.av[j]);
+            Acc::load(u + base + off, r.uv[j]);
+        } else {  // identity padding (Q3)
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) { r.av[j][k] = 1.0f; r.uv[j][k] = 0.0f; }
+        }
+    }
+    // ---- sequence heads -> reset pairs; A4 + A5
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+        long long s, t;
+        seq_pos(q0, r0, off, L, kTile, s, t);
+        if (t == 0 && base + off < total) {
+            const float hin = h0 ? __ldg(h0 + s) : 0.0f;
+            r.uv[j][0] = fmaf(r.av[j][0], hin, r.uv[j][0]);
+            r.av[j][0] = 0.0f;
+        }
+        row_scan(r, j, lane);
+    }
+    // ---- A6: cross-warp combine through shared memory
+    const Pair wt = warp_total(r);
+    if (lane == 0) s_warp[warp] = wt;
+    __syncthreads();
+    Pair X = identity_pair();  // composition of warps < warp
+    for (int w = 0; w < warp; ++w) X = compose(s_warp[w], X);
+
+    // ---- A7: decoupled look-back (warp 0)
+    if (warp == 0) {
+        Pair agg = s_warp[0];
+#pragma unroll
+        for (int w = 1; w < WARPS; ++w) agg = compose(s_warp[w], agg);
+        unsigned long long* my = desc + 2ull * tile;
+        const bool need_carry = (r0 != 0);  // a tile that starts at a head ignores its carry-in
+        const bool self_contained = (agg.P == 0.0f) || !need_carry;
+        if (lane == 0) {
+            if (self_contained) desc_store(my, kDescInclusive, Pair{0.0f, agg.U});
+            else desc_store(my, kDescAggregate, agg);
+        }
+        float h_in = 0.0f;
+        if (need_carry) {
+            Pair acc = identity_pair();  // (+) of the tiles examined so far (later side)
+            long long look = static_cast<long long>(tile) - 1;
+            while (true) {
+                const long long idx = look - lane;
+                Pair e{0.0f, 0.0f};
+                unsigned st = kDescInclusive;  // before the stream: state 0
+                if (idx >= 0) {
+                    const unsigned long long* d = desc + 2ull * idx;
+                    do { st = desc_load(d, e); } while (st == kDescEmpty);
+                }
+                __syncwarp();
+                const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);
+                const int first = incl ? (__ffs(incl) - 1) : 32;
+                if (lane > first) e = identity_pair();
+                // ordered tree reduction: lane 0 holds the LATEST tile (left operand)
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const Pair o = shfl_down_pair(e, d);
+                    if (lane + d < 32) e = compose(e, o);
+                }
+                const Pair win = shfl_pair(e, 0);
+                acc = compose(acc, win);
+                if (incl) break;
+                look -= 32;
+            }
+            h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
+            if (lane == 0 && !self_contained)
+                desc_store(my, kDescInclusive, Pair{0.0f, apply(agg, h_in)});
+        }
+        if (lane == 0) s_hin = h_in;
+    }
+    __syncthreads();
+
+    // ---- A8: apply the prefix and rescan the thread's steps; store h, h_last
+    float H = apply(X, s_hin);  // state entering this warp's slice
+#pragma unroll
+    for (int j = 0; j < J; ++j) {
+        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+        float hs = apply(r.excl[j], H);
+        float out[VEC];
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) {
+            hs = fmaf(r.av[j][k], hs, r.uv[j][k]);
+            out[k] = hs;
+        }
+        if (base + off < total) {
+            Acc::store(h + base + off, out);
+            if (h_last) {
+                long long s, t;
+                seq_pos(q0, r0, off, L, kTile, s, t);
+                if (t + VEC == L) h_last[s] = hs;
+            }
+        }
+        H = apply(r.tot[j], H);
+    }
+}
+
+// ====================================================================================
+// Variant AFFINESCAN_AFFINE_CTA_LOOP: one CTA per sequence, carry in a register (A7-i)
+// ====================================================================================
+template <typename T, int VEC, int J, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+affine_scan_cta_loop_kernel(const T* __restrict__ a, const T* __restrict__ u,
+                            const float* __restrict__ h0, T* __restrict__ h,
+                            float* __restrict__ h_last, long long num_seq, long long L)
+{
+    constexpr int kWarpElems = 32 * VEC * J;
+    constexpr int kTile = WARPS * kWarpElems;
+    using Acc = Access<T, VEC, true>;
+    __shared__ Pair s_warp[2][WARPS];
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+
+    for (long long s = blockIdx.x; s < num_seq; s += gridDim.x) {
+        const T* as = a + s * L;
+        const T* us = u + s * L;
+        T* hs_out = h + s * L;
+        float carry = h0 ? __ldg(h0 + s) : 0.0f;
+        int buf = 0;
+        for (long long t0 = 0; t0 < L; t0 += kTile, buf ^= 1) {
+            TileRegs<VEC, J> r;
+#pragma unroll
+            for (int j = 0; j < J; ++j) {
+                const long long t = t0 + warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                if (t < L) {
+                    Acc::load(as + t, r.av[j]);
+                    Acc::load(us + t, r.uv[j]);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) { r.av[j][k] = 1.0f; r.uv[j][k] = 0.0f; }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < J; ++j) row_scan(r, j, lane);
+            Pair X = identity_pair();
+            Pair agg = warp_total(r);
+            if (WARPS > 1) {
+                if (lane == 0) s_warp[buf][warp] = agg;
+                __syncthreads();  // one barrier per tile: s_warp is double-buffered
+                agg = s_warp[buf][0];
+#pragma unroll
+                for (int w = 1; w < WARPS; ++w) {
+                    if (w == warp) X = agg;
+                    agg = compose(s_warp[buf][w], agg);
+                }
+            }
+            float H = apply(X, carry);
+#pragma unroll
+            for (int j = 0; j < J; ++j) {
+                const long long t = t0 + warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                float hv = apply(r.excl[j], H);
+                float out[VEC];
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    hv = fmaf(r.av[j][k], hv, r.uv[j][k]);
+                    out[k] = hv;
+                }
+                if (t < L) Acc::store(hs_out + t, out);
+                H = apply(r.tot[j], H);
+            }
+            carry = apply(agg, carry);
+        }
+        if (h_last && threadIdx.x == 0) h_last[s] = carry;
+    }
+}
+
+// ====================================================================================
+// Variant AFFINESCAN_AFFINE_BLELLOCH (ABLATION): the paper's schedule (P:103-107,
+// P:163-167; Q3/Q4/Q16) on a shared-memory tile of 2*THREADS pairs:
+// upsweep (tree reduction), root <- (1,0), downsweep (prefix propagation), affine-prefix
+// reconstruction incl_t = e_t (+) excl_t, h_t = A_incl*carry + U_incl; CTA-loop carry.
+// Deliberately textbook: 2*log2(tile) barriers per tile and strided (bank-conflicting)
+// tree accesses are exactly the overheads the paper names.
+// ====================================================================================
+template <typename T, int THREADS>
+__global__ void __launch_bounds__(THREADS)
+affine_scan_blelloch_kernel(const T* __restrict__ a, const T* __restrict__ u,
+                            const float* __restrict__ h0, T* __restrict__ h,
+                            float* __restrict__ h_last, long long num_seq, long long L)
+{
+    constexpr int kTile = 2 * THREADS;
+    using Acc = Access<T, 1, false>;
+    __shared__ float sP[kTile];
+    __shared__ float sU[kTile];
+    __shared__ Pair s_total;
+    const int tid = threadIdx.x;
+
+    for (long long s = blockIdx.x; s < num_seq; s += gridDim.x) {
+        const T* as = a + s * L;
+        const T* us = u + s * L;
+        T* ho = h + s * L;
+        float carry = h0 ? __ldg(h0 + s) : 0.0f;
+        for (long long t0 = 0; t0 < L; t0 += kTile) {
+            float ea[2], eu[2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {  // shared-memory staging of the pairs
+                const long long t = t0 + tid + i * THREADS;
+                float va[1] = {1.0f}, vu[1] = {0.0f};  // identity padding (Q3)
+                if (t < L) { Acc::load(as + t, va); Acc::load(us + t, vu); }
+                ea[i] = va[0]; eu[i] = vu[0];
+                sP[tid + i * THREADS] = ea[i];
+                sU[tid + i * THREADS] = eu[i];
+            }
+            // upsweep: x[r] <- x[r] (+) x[l], r later
+            for (int stride = 1; stride < kTile; stride <<= 1) {
+                __syncthreads();
+                const int rr = (tid + 1) * 2 * stride - 1;
+                if (rr < kTile) {
+                    const int ll = rr - stride;
+                    const Pair v = compose(Pair{sP[rr], sU[rr]}, Pair{sP[ll], sU[ll]});
+                    sP[rr] = v.P; sU[rr] = v.U;
+                }
+            }
+            __syncthreads();
+            if (tid == 0) {  // root initialisation: keep the total, root <- identity
+                s_total = Pair{sP[kTile - 1], sU[kTile - 1]};
+                sP[kTile - 1] = 1.0f; sU[kTile - 1] = 0.0f;
+            }
+            // downsweep: t <- x[l]; x[l] <- x[r]; x[r] <- t (+) x[r]_old
+            for (int stride = kTile >> 1; stride >= 1; stride >>= 1) {
+                __syncthreads();
+                const int rr = (tid + 1) * 2 * stride - 1;
+                if (rr < kTile) {
+                    const int ll = rr - stride;
+                    const Pair left{sP[ll], sU[ll]};
+                    const Pair inh{sP[rr], sU[rr]};
+                    sP[ll] = inh.P; sU[ll] = inh.U;
+                    const Pair v = compose(left, inh);
+                    sP[rr] = v.P; sU[rr] = v.U;
+                }
+            }
+            __syncthreads();
+            // affine-prefix reconstruction
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int idx = tid + i * THREADS;
+                const long long t = t0 + idx;
+                const Pair incl = compose(Pair{ea[i], eu[i]}, Pair{sP[idx], sU[idx]});
+                float out[1] = {apply(incl, carry)};
+                if (t < L) Acc::store(ho + t, out);
+            }
+            carry = apply(s_total, carry);
+            __syncthreads();  // smem tile and s_total are reused by the next tile
+        }
+        if (h_last && tid == 0) h_last[s] = carry;
+    }
+}
+
+}  // namespace affinescan

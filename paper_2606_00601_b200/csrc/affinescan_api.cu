@@ -1,0 +1,495 @@
+// affinescan_api.cu — C-ABI boundary and host launch layer of libaffinescan
+// (include/affinescan.h).  Validates arguments, picks a kernel variant from the shape,
+// and enqueues the kernels on the caller's stream.  No torch types, no exceptions.
+#include "../../include/affinescan.h"
+
+#include <atomic>
+#include <cstdint>
+#include <limits>
+#include <map>
+#include <mutex>
+#include <utility>
+#include <vector>
+
+#include "affine_scan.cuh"
+#include "selective_scan_lane_row.cuh"
+#include "selective_scan_warp_row.cuh"
+
+namespace {
+
+using namespace affinescan;
+using bf16 = __nv_bfloat16;
+
+thread_local int tl_last_cuda_error = 0;
+thread_local int tl_last_variant = 0;
+std::atomic<int64_t> g_launches{0};
+
+int cuda_fail(cudaError_t e)
+{
+    tl_last_cuda_error = static_cast<int>(e);
+    (void)cudaGetLastError();  // clear the sticky-less error state
+    return AFFINESCAN_ERR_CUDA;
+}
+#define AS_CUDA(call)                                     \
+    do {                                                  \
+        const cudaError_t e__ = (call);                   \
+        if (e__ != cudaSuccess) return cuda_fail(e__);    \
+    } while (0)
+
+int after_launch()
+{
+    g_launches.fetch_add(1, std::memory_order_relaxed);
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? AFFINESCAN_OK : cuda_fail(e);
+}
+
+bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+
+bool mul_overflows(int64_t a, int64_t b, int64_t* out)
+{
+    return __builtin_mul_overflow(a, b, out);
+}
+
+// ---------------------------------------------------------------- device buffer caches
+struct Buffer {
+    void* ptr = nullptr;
+    size_t bytes = 0;
+};
+std::mutex g_mu;
+std::map<std::pair<int, void*>, Buffer> g_scratch;  // (device, stream) -> look-back scratch
+std::map<std::pair<int, int>, Buffer> g_staging;    // (device, slot)   -> host-API staging
+
+int grow(Buffer& b, size_t bytes)
+{
+    if (b.bytes >= bytes) return AFFINESCAN_OK;
+    if (b.ptr) {
+        AS_CUDA(cudaDeviceSynchronize());  // an earlier call on this stream may still use it
+        AS_CUDA(cudaFree(b.ptr));
+        b.ptr = nullptr;
+        b.bytes = 0;
+    }
+    const size_t want = bytes + bytes / 4 + 256;
+    AS_CUDA(cudaMalloc(&b.ptr, want));
+    b.bytes = want;
+    return AFFINESCAN_OK;
+}
+
+int get_scratch(cudaStream_t stream, size_t bytes, void** out)
+{
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_mu);
+    Buffer& b = g_scratch[{dev, static_cast<void*>(stream)}];
+    const int st = grow(b, bytes);
+    if (st != AFFINESCAN_OK) return st;
+    *out = b.ptr;
+    return AFFINESCAN_OK;
+}
+
+int get_staging(int slot, size_t bytes, void** out)
+{
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_mu);
+    Buffer& b = g_staging[{dev, slot}];
+    const int st = grow(b, bytes ? bytes : 1);
+    if (st != AFFINESCAN_OK) return st;
+    *out = b.ptr;
+    return AFFINESCAN_OK;
+}
+
+size_t elt_size(int io_dtype) { return io_dtype == AFFINESCAN_BF16 ? 2 : 4; }
+
+// ============================================================== affine_scan dispatch
+constexpr int kAffJ = 4;       // 128-bit vectors per thread per tile
+constexpr int kAffWarps = 8;   // 256 threads
+
+template <typename T, int VEC>
+int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float* h_last,
+                           int64_t num_seq, int64_t L, cudaStream_t stream)
+{
+    constexpr int kTile = kAffWarps * 32 * VEC * kAffJ;
+    const int64_t total = num_seq * L;
+    const int64_t ntiles = (total + kTile - 1) / kTile;
+    if (ntiles > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    void* scratch = nullptr;
+    const size_t desc_bytes = static_cast<size_t>(ntiles) * 16;
+    const int st = get_scratch(stream, desc_bytes + 16, &scratch);
+    if (st != AFFINESCAN_OK) return st;
+    AS_CUDA(cudaMemsetAsync(scratch, 0, desc_bytes + 16, stream));
+    auto* desc = static_cast<unsigned long long*>(scratch);
+    auto* ticket = reinterpret_cast<unsigned*>(static_cast<unsigned char*>(scratch) + desc_bytes);
+    affine_scan_lookback_kernel<T, VEC, kAffJ, kAffWarps>
+        <<<static_cast<unsigned>(ntiles), kAffWarps * 32, 0, stream>>>(a, u, h0, h, h_last, total, L,
+                                                                      desc, ticket);
+    return after_launch();
+}
+
+template <typename T, int VEC>
+int launch_affine_cta_loop(const T* a, const T* u, const float* h0, T* h, float* h_last,
+                           int64_t num_seq, int64_t L, cudaStream_t stream)
+{
+    const unsigned grid = static_cast<unsigned>(num_seq < 0x7fffffffLL ? num_seq : 0x7fffffffLL);
+    // short sequences: one warp per CTA keeps every lane busy; long ones: 8 warps per tile
+    if (L <= static_cast<int64_t>(32 * VEC * kAffJ) * 2) {
+        affine_scan_cta_loop_kernel<T, VEC, kAffJ, 1><<<grid, 32, 0, stream>>>(a, u, h0, h, h_last,
+                                                                                num_seq, L);
+    } else {
+        affine_scan_cta_loop_kernel<T, VEC, kAffJ, kAffWarps>
+            <<<grid, kAffWarps * 32, 0, stream>>>(a, u, h0, h, h_last, num_seq, L);
+    }
+    return after_launch();
+}
+
+template <typename T>
+int launch_affine_blelloch(const T* a, const T* u, const float* h0, T* h, float* h_last,
+                           int64_t num_seq, int64_t L, cudaStream_t stream)
+{
+    const unsigned grid = static_cast<unsigned>(num_seq < 0x7fffffffLL ? num_seq : 0x7fffffffLL);
+    affine_scan_blelloch_kernel<T, 512><<<grid, 512, 0, stream>>>(a, u, h0, h, h_last, num_seq, L);
+    return after_launch();
+}
+
+template <typename T>
+int affine_dispatch(const void* a_, const void* u_, const float* h0, void* h_, float* h_last,
+                    int64_t num_seq, int64_t L, int variant, cudaStream_t stream)
+{
+    const T* a = static_cast<const T*>(a_);
+    const T* u = static_cast<const T*>(u_);
+    T* h = static_cast<T*>(h_);
+    constexpr int kVec = Io<T>::kVec;
+    const bool vec_ok = (L % kVec == 0) && aligned16(a) && aligned16(u) && aligned16(h);
+    if (variant == AFFINESCAN_VARIANT_AUTO) variant = AFFINESCAN_AFFINE_LOOKBACK;
+    int st;
+    switch (variant) {
+    case AFFINESCAN_AFFINE_LOOKBACK:
+        st = vec_ok ? launch_affine_lookback<T, kVec>(a, u, h0, h, h_last, num_seq, L, stream)
+                    : launch_affine_lookback<T, 1>(a, u, h0, h, h_last, num_seq, L, stream);
+        break;
+    case AFFINESCAN_AFFINE_CTA_LOOP:
+        st = vec_ok ? launch_affine_cta_loop<T, kVec>(a, u, h0, h, h_last, num_seq, L, stream)
+                    : launch_affine_cta_loop<T, 1>(a, u, h0, h, h_last, num_seq, L, stream);
+        break;
+    case AFFINESCAN_AFFINE_BLELLOCH:
+        st = launch_affine_blelloch<T>(a, u, h0, h, h_last, num_seq, L, stream);
+        break;
+    default:
+        return AFFINESCAN_ERR_UNSUPPORTED;
+    }
+    if (st == AFFINESCAN_OK) tl_last_variant = variant;
+    return st;
+}
+
+__global__ void fill_h_last_kernel(const float* __restrict__ h0, float* __restrict__ h_last,
+                                   long long n)
+{
+    const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i < n) h_last[i] = h0 ? h0[i] : 0.0f;
+}
+
+int fill_h_last(const float* h0, float* h_last, int64_t n, cudaStream_t stream)
+{
+    if (!h_last || n <= 0) return AFFINESCAN_OK;
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    fill_h_last_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(h0, h_last, n);
+    return after_launch();
+}
+
+int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, float* h_last,
+                     int64_t num_seq, int64_t L, int io_dtype, int variant, void* cuda_stream)
+{
+    tl_last_variant = 0;
+    if (io_dtype != AFFINESCAN_F32 && io_dtype != AFFINESCAN_BF16) return AFFINESCAN_ERR_DTYPE;
+    if (num_seq < 0 || L < 0) return AFFINESCAN_ERR_SHAPE;
+    int64_t total = 0;
+    if (mul_overflows(num_seq, L, &total) || total > (std::numeric_limits<int64_t>::max() >> 3))
+        return AFFINESCAN_ERR_SHAPE;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (num_seq == 0) return AFFINESCAN_OK;
+    if (L == 0) return fill_h_last(h0, h_last, num_seq, stream);  // h_last <- h0 (or 0)
+    if (!a || !u || !h) return AFFINESCAN_ERR_NULL;
+    return io_dtype == AFFINESCAN_F32
+               ? affine_dispatch<float>(a, u, h0, h, h_last, num_seq, L, variant, stream)
+               : affine_dispatch<bf16>(a, u, h0, h, h_last, num_seq, L, variant, stream);
+}
+
+// ============================================================== selective_scan dispatch
+constexpr int kSelWarps = 4;        // warp_row: rows per CTA
+constexpr int kLaneRowTc = 64;      // lane_row: timesteps per staged B/C tile
+constexpr int kLaneRowWarps = 4;    // lane_row: 128 rows per CTA
+constexpr int64_t kLaneRowMinRows = 148 * 32 * 4;  // one row per FP32 lane of the machine
+
+template <typename T, int VEC, int NV>
+int launch_warp_row(const T* x, const T* delta, const float* A, const T* B, const T* C,
+                    const float* D, const float* h0, T* y, float* h_last, int batch, int d_inner,
+                    int N, int64_t L, cudaStream_t stream)
+{
+    const int64_t rows = static_cast<int64_t>(batch) * d_inner;
+    const int64_t blocks = (rows + kSelWarps - 1) / kSelWarps;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    selective_scan_warp_row_kernel<T, VEC, NV, kSelWarps>
+        <<<static_cast<unsigned>(blocks), kSelWarps * 32, 0, stream>>>(x, delta, A, B, C, D, h0, y,
+                                                                       h_last, batch, d_inner, N, L);
+    return after_launch();
+}
+
+template <typename T>
+int launch_lane_row(const T* x, const T* delta, const float* A, const T* B, const T* C,
+                    const float* D, const float* h0, T* y, float* h_last, int batch, int d_inner,
+                    int64_t L, cudaStream_t stream)
+{
+    using S = LaneRowSmem<T, kLaneRowTc>;
+    auto kern = selective_scan_lane_row_kernel<T, kLaneRowTc, kLaneRowWarps>;
+    constexpr int smem = S::kPerWarp * kLaneRowWarps;
+    static std::atomic<unsigned> configured{0};  // bit per device
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    if (!(configured.load() & (1u << (dev & 31)))) {
+        AS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        configured.fetch_or(1u << (dev & 31));
+    }
+    const int64_t rows = static_cast<int64_t>(batch) * d_inner;
+    const int64_t warps = rows / 32;
+    const int64_t blocks = (warps + kLaneRowWarps - 1) / kLaneRowWarps;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    kern<<<static_cast<unsigned>(blocks), kLaneRowWarps * 32, smem, stream>>>(
+        x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, L);
+    return after_launch();
+}
+
+template <typename T>
+int selective_dispatch(const void* x_, const void* delta_, const float* A, const void* B_,
+                       const void* C_, const float* D, const float* h0, void* y_, float* h_last,
+                       int batch, int d_inner, int N, int64_t L, int variant, cudaStream_t stream)
+{
+    const T* x = static_cast<const T*>(x_);
+    const T* delta = static_cast<const T*>(delta_);
+    const T* B = static_cast<const T*>(B_);
+    const T* C = static_cast<const T*>(C_);
+    T* y = static_cast<T*>(y_);
+    constexpr int kVec = Io<T>::kVec;
+    const bool vec_ok = (L % kVec == 0) && aligned16(x) && aligned16(delta) && aligned16(B) &&
+                        aligned16(C) && aligned16(y);
+    const bool lane_ok = vec_ok && N == 16 && (d_inner % 32 == 0) && aligned16(A) &&
+                         (!h0 || aligned16(h0)) && (!h_last || aligned16(h_last));
+    const int64_t rows = static_cast<int64_t>(batch) * d_inner;
+    if (variant == AFFINESCAN_VARIANT_AUTO)
+        variant = (lane_ok && rows >= kLaneRowMinRows) ? AFFINESCAN_SELECTIVE_LANE_ROW
+                                                       : AFFINESCAN_SELECTIVE_WARP_ROW;
+    int st;
+    switch (variant) {
+    case AFFINESCAN_SELECTIVE_WARP_ROW:
+        if (vec_ok)
+            st = launch_warp_row<T, kVec, 16 / kVec>(x, delta, A, B, C, D, h0, y, h_last, batch,
+                                                     d_inner, N, L, stream);
+        else
+            st = launch_warp_row<T, 1, 4>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, N, L,
+                                          stream);
+        break;
+    case AFFINESCAN_SELECTIVE_LANE_ROW:
+        if (!lane_ok) return AFFINESCAN_ERR_UNSUPPORTED;
+        st = launch_lane_row<T>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, L, stream);
+        break;
+    default:
+        return AFFINESCAN_ERR_UNSUPPORTED;
+    }
+    if (st == AFFINESCAN_OK) tl_last_variant = variant;
+    return st;
+}
+
+int selective_scan_impl(const void* x, const void* delta, const float* A, const void* B,
+                        const void* C, const float* D, const float* h0, void* y, float* h_last,
+                        int batch, int d_inner, int N, int64_t L, int io_dtype, int variant,
+                        void* cuda_stream)
+{
+    tl_last_variant = 0;
+    if (io_dtype != AFFINESCAN_F32 && io_dtype != AFFINESCAN_BF16) return AFFINESCAN_ERR_DTYPE;
+    if (batch < 0 || d_inner < 0 || L < 0) return AFFINESCAN_ERR_SHAPE;
+    if (N < 1 || N > AFFINESCAN_MAX_N) return AFFINESCAN_ERR_UNSUPPORTED;
+    int64_t rows = 0, total = 0, bnl = 0;
+    if (mul_overflows(batch, d_inner, &rows) || mul_overflows(rows, L, &total) ||
+        mul_overflows(static_cast<int64_t>(batch) * N, L, &bnl) ||
+        total > (std::numeric_limits<int64_t>::max() >> 3) ||
+        bnl > (std::numeric_limits<int64_t>::max() >> 3))
+        return AFFINESCAN_ERR_SHAPE;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (rows == 0) return AFFINESCAN_OK;
+    if (L == 0) return fill_h_last(h0, h_last, rows * N, stream);
+    if (!x || !delta || !A || !B || !C || !y) return AFFINESCAN_ERR_NULL;
+    return io_dtype == AFFINESCAN_F32
+               ? selective_dispatch<float>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, N,
+                                           L, variant, stream)
+               : selective_dispatch<bf16>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, N,
+                                          L, variant, stream);
+}
+
+// ---------------------------------------------------------------- host-buffer helpers
+struct Staged {
+    void* dev = nullptr;
+};
+
+int stage_in(int slot, const void* host, size_t bytes, cudaStream_t stream, void** dev)
+{
+    *dev = nullptr;
+    if (!host) return AFFINESCAN_OK;
+    const int st = get_staging(slot, bytes, dev);
+    if (st != AFFINESCAN_OK) return st;
+    if (bytes) AS_CUDA(cudaMemcpyAsync(*dev, host, bytes, cudaMemcpyHostToDevice, stream));
+    return AFFINESCAN_OK;
+}
+
+int stage_out_alloc(int slot, const void* host, size_t bytes, void** dev)
+{
+    *dev = nullptr;
+    if (!host) return AFFINESCAN_OK;
+    return get_staging(slot, bytes, dev);
+}
+
+}  // namespace
+
+// =================================================================== exported C ABI
+extern "C" {
+
+int affine_scan(const void* a, const void* u, const float* h0, void* h, float* h_last,
+                int64_t num_seq, int64_t L, int io_dtype, void* cuda_stream)
+{
+    return affine_scan_impl(a, u, h0, h, h_last, num_seq, L, io_dtype, AFFINESCAN_VARIANT_AUTO,
+                            cuda_stream);
+}
+
+int affine_scan_ex(const void* a, const void* u, const float* h0, void* h, float* h_last,
+                   int64_t num_seq, int64_t L, int io_dtype, int variant, void* cuda_stream)
+{
+    return affine_scan_impl(a, u, h0, h, h_last, num_seq, L, io_dtype, variant, cuda_stream);
+}
+
+int affine_scan_host(const void* a, const void* u, const float* h0, void* h, float* h_last,
+                     int64_t num_seq, int64_t L, int io_dtype, void* cuda_stream)
+{
+    if (io_dtype != AFFINESCAN_F32 && io_dtype != AFFINESCAN_BF16) return AFFINESCAN_ERR_DTYPE;
+    if (num_seq < 0 || L < 0) return AFFINESCAN_ERR_SHAPE;
+    int64_t total = 0;
+    if (mul_overflows(num_seq, L, &total) || total > (std::numeric_limits<int64_t>::max() >> 3))
+        return AFFINESCAN_ERR_SHAPE;
+    if (total > 0 && (!a || !u || !h)) return AFFINESCAN_ERR_NULL;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const size_t eb = static_cast<size_t>(total) * elt_size(io_dtype);
+    const size_t sb = static_cast<size_t>(num_seq) * sizeof(float);
+    void *da, *du, *dh0, *dh, *dhl;
+    int st;
+    if ((st = stage_in(0, a, eb, stream, &da)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(1, u, eb, stream, &du)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(2, h0, sb, stream, &dh0)) != AFFINESCAN_OK) return st;
+    if ((st = stage_out_alloc(3, h, eb, &dh)) != AFFINESCAN_OK) return st;
+    if ((st = stage_out_alloc(4, h_last, sb, &dhl)) != AFFINESCAN_OK) return st;
+    st = affine_scan_impl(da, du, static_cast<const float*>(dh0), dh, static_cast<float*>(dhl),
+                          num_seq, L, io_dtype, AFFINESCAN_VARIANT_AUTO, cuda_stream);
+    if (st != AFFINESCAN_OK) return st;
+    if (h && eb) AS_CUDA(cudaMemcpyAsync(h, dh, eb, cudaMemcpyDeviceToHost, stream));
+    if (h_last && sb) AS_CUDA(cudaMemcpyAsync(h_last, dhl, sb, cudaMemcpyDeviceToHost, stream));
+    AS_CUDA(cudaStreamSynchronize(stream));
+    return AFFINESCAN_OK;
+}
+
+int selective_scan_fwd(const void* x, const void* delta, const float* A, const void* B,
+                       const void* C, const float* D, const float* h0, void* y, float* h_last,
+                       int batch, int d_inner, int N, int64_t L, int io_dtype, void* cuda_stream)
+{
+    return selective_scan_impl(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, N, L, io_dtype,
+                               AFFINESCAN_VARIANT_AUTO, cuda_stream);
+}
+
+int selective_scan_fwd_ex(const void* x, const void* delta, const float* A, const void* B,
+                          const void* C, const float* D, const float* h0, void* y, float* h_last,
+                          int batch, int d_inner, int N, int64_t L, int io_dtype, int variant,
+                          void* cuda_stream)
+{
+    return selective_scan_impl(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, N, L, io_dtype,
+                               variant, cuda_stream);
+}
+
+int selective_scan_fwd_host(const void* x, const void* delta, const float* A, const void* B,
+                            const void* C, const float* D, const float* h0, void* y, float* h_last,
+                            int batch, int d_inner, int N, int64_t L, int io_dtype,
+                            void* cuda_stream)
+{
+    if (io_dtype != AFFINESCAN_F32 && io_dtype != AFFINESCAN_BF16) return AFFINESCAN_ERR_DTYPE;
+    if (batch < 0 || d_inner < 0 || L < 0) return AFFINESCAN_ERR_SHAPE;
+    if (N < 1 || N > AFFINESCAN_MAX_N) return AFFINESCAN_ERR_UNSUPPORTED;
+    int64_t rows = 0, total = 0, bnl = 0;
+    if (mul_overflows(batch, d_inner, &rows) || mul_overflows(rows, L, &total) ||
+        mul_overflows(static_cast<int64_t>(batch) * N, L, &bnl) ||
+        total > (std::numeric_limits<int64_t>::max() >> 3) ||
+        bnl > (std::numeric_limits<int64_t>::max() >> 3))
+        return AFFINESCAN_ERR_SHAPE;
+    if (total > 0 && (!x || !delta || !A || !B || !C || !y)) return AFFINESCAN_ERR_NULL;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const size_t es = elt_size(io_dtype);
+    const size_t xb = static_cast<size_t>(total) * es;
+    const size_t bb = static_cast<size_t>(bnl) * es;
+    const size_t ab = static_cast<size_t>(d_inner) * N * sizeof(float);
+    const size_t db = static_cast<size_t>(d_inner) * sizeof(float);
+    const size_t hb = static_cast<size_t>(rows) * N * sizeof(float);
+    void *dx, *dd, *dA, *dB, *dC, *dD, *dh0, *dy, *dhl;
+    int st;
+    if ((st = stage_in(10, x, xb, stream, &dx)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(11, delta, xb, stream, &dd)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(12, A, ab, stream, &dA)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(13, B, bb, stream, &dB)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(14, C, bb, stream, &dC)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(15, D, db, stream, &dD)) != AFFINESCAN_OK) return st;
+    if ((st = stage_in(16, h0, hb, stream, &dh0)) != AFFINESCAN_OK) return st;
+    if ((st = stage_out_alloc(17, y, xb, &dy)) != AFFINESCAN_OK) return st;
+    if ((st = stage_out_alloc(18, h_last, hb, &dhl)) != AFFINESCAN_OK) return st;
+    st = selective_scan_impl(dx, dd, static_cast<const float*>(dA), dB, dC,
+                             static_cast<const float*>(dD), static_cast<const float*>(dh0), dy,
+                             static_cast<float*>(dhl), batch, d_inner, N, L, io_dtype,
+                             AFFINESCAN_VARIANT_AUTO, cuda_stream);
+    if (st != AFFINESCAN_OK) return st;
+    if (y && xb) AS_CUDA(cudaMemcpyAsync(y, dy, xb, cudaMemcpyDeviceToHost, stream));
+    if (h_last && hb) AS_CUDA(cudaMemcpyAsync(h_last, dhl, hb, cudaMemcpyDeviceToHost, stream));
+    AS_CUDA(cudaStreamSynchronize(stream));
+    return AFFINESCAN_OK;
+}
+
+const char* affinescan_status_string(int status)
+{
+    switch (status) {
+    case AFFINESCAN_OK: return "ok";
+    case AFFINESCAN_ERR_NULL: return "a required pointer is NULL";
+    case AFFINESCAN_ERR_SHAPE: return "negative or overflowing shape";
+    case AFFINESCAN_ERR_DTYPE: return "unknown io dtype";
+    case AFFINESCAN_ERR_UNSUPPORTED: return "unsupported N, variant or shape for the forced variant";
+    case AFFINESCAN_ERR_CUDA: return "CUDA runtime error (see affinescan_last_cuda_error)";
+    default: return "unknown status";
+    }
+}
+
+int affinescan_last_cuda_error(void) { return tl_last_cuda_error; }
+int affinescan_last_variant(void) { return tl_last_variant; }
+int64_t affinescan_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+int affinescan_version(void) { return 100; }
+
+int affinescan_release_cache(void)
+{
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    AS_CUDA(cudaDeviceSynchronize());
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (auto it = g_scratch.begin(); it != g_scratch.end();) {
+        if (it->first.first == dev) {
+            if (it->second.ptr) cudaFree(it->second.ptr);
+            it = g_scratch.erase(it);
+        } else ++it;
+    }
+    for (auto it = g_staging.begin(); it != g_staging.end();) {
+        if (it->first.first == dev) {
+            if (it->second.ptr) cudaFree(it->second.ptr);
+            it = g_staging.erase(it);
+        } else ++it;
+    }
+    return AFFINESCAN_OK;
+}
+
+}  // extern "C"

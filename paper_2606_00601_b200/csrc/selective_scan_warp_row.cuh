@@ -1,0 +1,154 @@
+// selective_scan_warp_row.cuh — variant AFFINESCAN_SELECTIVE_WARP_ROW of
+// selective_scan_fwd (include/affinescan.h; BJ north_star).
+//
+// One warp owns one (b,d) row.  A warp tile is 32*K consecutive timesteps: lane l owns
+// the K consecutive steps [l*K, l*K+K).  For each state n (outer loop) the lane
+//   A3  discretises      a_k = ex2(delta_k * A2[n]),  u_k = (delta_k x_k) * B_k[n]
+//   A4  composes its K pairs in registers (P via one ex2 of A2[n]*sum(delta))
+//   A5  combines across the warp with a Kogge–Stone __shfl_up_sync pair scan
+//   A7  takes the carry h_in[n] of the previous tile (CTA-loop style, in a register)
+//   A8  rescans its K steps from the exclusive prefix (a_k, u_k still in registers)
+//   A9  accumulates y_k += C_k[n] * h_k ; h itself is never stored.
+// x/delta/B/C/y move with coalesced 128-bit accesses (lane owns K contiguous elements).
+// This is the schedule for few-row shapes (cfg2, cfg4) and the general fallback
+// (any N <= 64, any L, any alignment via the scalar-access instantiation).
+#pragma once
+
+#include "common.cuh"
+
+namespace affinescan {
+
+// NV vectors of VEC elements per lane: K = NV*VEC consecutive timesteps.
+template <typename T, int VEC, int NV, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
+                               const float* __restrict__ A, const T* __restrict__ B,
+                               const T* __restrict__ C, const float* __restrict__ D,
+                               const float* __restrict__ h0, T* __restrict__ y,
+                               float* __restrict__ h_last, int batch, int d_inner, int N,
+                               long long L)
+{
+    constexpr int K = NV * VEC;
+    constexpr int kWarpTile = 32 * K;
+    using AccS = Access<T, VEC, true>;   // streamed once: x, delta, y
+    using AccR = Access<T, VEC, false>;  // re-read by every row of the batch: B, C
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const long long rows = static_cast<long long>(batch) * d_inner;
+    const long long row = static_cast<long long>(blockIdx.x) * WARPS + warp;
+    if (row >= rows) return;
+    const int b = static_cast<int>(row / d_inner);
+    const int d = static_cast<int>(row - static_cast<long long>(b) * d_inner);
+
+    const T* xr = x + row * L;
+    const T* dr = delta + row * L;
+    T* yr = y + row * L;
+    const T* Bb = B + static_cast<long long>(b) * N * L;
+    const T* Cb = C + static_cast<long long>(b) * N * L;
+
+    // Lane n (and n+32) keeps A2[n] = A[d,n]*log2(e) and the carry h_in[n]; they are
+    // broadcast with one shuffle per (n, tile).
+    float A2r[2], hcr[2];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const int n = lane + 32 * i;
+        A2r[i] = n < N ? __ldg(A + static_cast<long long>(d) * N + n) * kLog2e : 0.0f;
+        hcr[i] = (n < N && h0) ? __ldg(h0 + row * N + n) : 0.0f;
+    }
+    const float Dd = D ? __ldg(D + d) : 0.0f;
+
+    for (long long t0 = 0; t0 < L; t0 += kWarpTile) {
+        const long long tl = t0 + lane * K;  // first timestep of this lane
+        float dl[K], dx[K], yv[K];
+        // ---- A1: x, delta
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            float xv[VEC], dv[VEC];
+            if (tl + v * VEC < L) {
+                AccS::load(xr + tl + v * VEC, xv);
+                AccS::load(dr + tl + v * VEC, dv);
+            } else {  // identity padding: delta = 0 => a = 1, u = 0 (Q12)
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) { xv[k] = 0.0f; dv[k] = 0.0f; }
+            }
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) {
+                dl[v * VEC + k] = dv[k];
+                dx[v * VEC + k] = dv[k] * xv[k];
+                yv[v * VEC + k] = Dd * xv[k];
+            }
+        }
+        float dsum = 0.0f;
+#pragma unroll
+        for (int k = 0; k < K; ++k) dsum += dl[k];
+
+        for (int n = 0; n < N; ++n) {
+            const bool hi = n >= 32;  // explicit selects: no dynamic register indexing
+            const float A2n = __shfl_sync(kFullMask, hi ? A2r[1] : A2r[0], n & 31);
+            const float hin = __shfl_sync(kFullMask, hi ? hcr[1] : hcr[0], n & 31);
+            const T* Bn = Bb + static_cast<long long>(n) * L;
+            const T* Cn = Cb + static_cast<long long>(n) * L;
+            float a[K], u[K], cv[K];
+            // ---- A2 (B_t, C_t) + A3 (discretise)
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                float bv[VEC], cc[VEC];
+                if (tl + v * VEC < L) {
+                    AccR::load(Bn + tl + v * VEC, bv);
+                    AccR::load(Cn + tl + v * VEC, cc);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) { bv[k] = 0.0f; cc[k] = 0.0f; }
+                }
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    a[v * VEC + k] = ex2_approx(dl[v * VEC + k] * A2n);
+                    u[v * VEC + k] = dx[v * VEC + k] * bv[k];
+                    cv[v * VEC + k] = cc[k];
+                }
+            }
+            // ---- A4: thread-local composition of K pairs
+            Pair loc{ex2_approx(dsum * A2n), u[0]};
+#pragma unroll
+            for (int k = 1; k < K; ++k) loc.U = fmaf(a[k], loc.U, u[k]);
+            // ---- A5: warp combine
+            const Pair inc = warp_inclusive_scan(loc, lane);
+            Pair ex = shfl_up_pair(inc, 1);
+            if (lane == 0) ex = identity_pair();
+            const Pair tot = shfl_pair(inc, 31);
+            // ---- A7/A8: carry-in, rescan; A9: y accumulation
+            float hv = apply(ex, hin);
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                hv = fmaf(a[k], hv, u[k]);
+                yv[k] = fmaf(cv[k], hv, yv[k]);
+            }
+            const float hout = apply(tot, hin);  // state after the tile (uniform)
+            if ((n & 31) == lane) {
+                if (hi) hcr[1] = hout;
+                else hcr[0] = hout;
+            }
+        }
+        // ---- A9: store y
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            if (tl + v * VEC < L) {
+                float out[VEC];
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) out[k] = yv[v * VEC + k];
+                AccS::store(yr + tl + v * VEC, out);
+            }
+        }
+    }
+    // ---- A10: final state
+    if (h_last) {
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const int n = lane + 32 * i;
+            if (n < N) h_last[row * N + n] = hcr[i];
+        }
+    }
+}
+
+}  // namespace affinescan

@@ -1,0 +1,416 @@
+"""GPU parity tests: the CUDA path (through the C-ABI, via the ctypes binding) against the
+float64 CPU oracle, element by element, on the same seeded inputs.
+
+Tolerances are BASELINE.json's: max|err| <= 1e-4*(1+|ref|) for fp32 io and
+2e-2*(1+|ref|) for bf16 io with fp32 state.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import paper_2606_00601_b200 as lib
+from workloads import (config, make_affine_inputs, make_selective_inputs, normal, to_f64_numpy,
+                       uniform)
+
+from util import (TOL, assert_close, check_affine, check_selective, gpu_affine, gpu_selective,
+                  lane_row_ok, oracle_affine, oracle_selective, oracle_selective_rows, rel_err)
+
+pytestmark = pytest.mark.gpu
+
+AFFINE_VARIANTS = [lib.AFFINE_LOOKBACK, lib.AFFINE_CTA_LOOP, lib.AFFINE_BLELLOCH]
+DTYPES = [torch.float32, torch.bfloat16]
+
+
+def _affine_inputs(S, L, dtype, dev, seed, with_h0=True, a_lo=0.5, a_hi=0.99):
+    a = uniform((S, L), a_lo, a_hi, seed=seed, stream=0, device=dev, dtype=dtype)
+    u = normal((S, L), seed=seed, stream=1, device=dev, dtype=dtype)
+    h0 = normal((S,), seed=seed, stream=2, device=dev, dtype=torch.float32) if with_h0 else None
+    return {"a": a, "u": u, "h0": h0}
+
+
+def _selective_inputs(batch, d_inner, N, L, dtype, dev, seed, with_D=True, with_h0=False,
+                      delta_shift=-2.0):
+    c = config(2, batch=batch, d_inner=d_inner, N=N, L=L, dtype=dtype, delta_shift=delta_shift,
+               seed=seed)
+    inp = make_selective_inputs(c, device=dev, with_h0=with_h0)
+    if not with_D:
+        inp["D"] = None
+    return inp
+
+
+# =============================================================== affine_scan: T1 shapes
+@pytest.mark.parametrize("variant", AFFINE_VARIANTS)
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_affine_small_and_ragged_shapes(cuda_device, variant, dtype):
+    """Tiny, odd and ragged shapes spanning several tiles, vector and scalar paths."""
+    Ls = [1, 2, 3, 4, 5, 8, 31, 32, 33, 127, 128, 255, 256, 257, 511, 512, 1023, 1024, 1025,
+          2047, 2048, 2049, 4095, 4096, 4100, 8191, 8200, 12296]
+    seed = 100
+    for L in Ls:
+        for S in (1, 3, 33):
+            if S * L > 300_000:
+                continue
+            seed += 1
+            inp = _affine_inputs(S, L, dtype, cuda_device, seed, with_h0=(seed % 2 == 0))
+            check_affine(inp, variant, f"S={S} L={L} {dtype} v={variant}")
+
+
+@pytest.mark.parametrize("variant", AFFINE_VARIANTS)
+def test_affine_long_sequences_cross_many_tiles(cuda_device, variant):
+    for (S, L) in [(2, 65536 + 4), (1, 262144), (5, 40000)]:
+        inp = _affine_inputs(S, L, torch.float32, cuda_device, 7 + L, a_lo=0.9, a_hi=0.9999)
+        check_affine(inp, variant, f"S={S} L={L}")
+
+
+@pytest.mark.parametrize("variant", AFFINE_VARIANTS)
+def test_affine_prefix_sum_exact_through_the_whole_carry_chain(cuda_device, variant):
+    """a≡1 (BJ closed form): P never reaches 0, so every tile's carry really depends on all
+    its predecessors; u in {0,1} keeps every partial sum an exact fp32 integer."""
+    S, L = 2, 1 << 20
+    u = (uniform((S, L), 0, 1, seed=5, stream=0, device=cuda_device) > 0.5).to(torch.float32)
+    inp = {"a": torch.ones_like(u), "u": u,
+           "h0": torch.tensor([3.0, -7.0], device=cuda_device)}
+    h, h_last = gpu_affine(inp, variant)
+    ref = inp["h0"].double()[:, None] + torch.cumsum(u.double(), dim=1)
+    assert torch.equal(h.double(), ref)
+    assert torch.equal(h_last.double(), ref[:, -1])
+    href, _ = oracle_affine({"a": inp["a"][:, :4096], "u": u[:, :4096], "h0": inp["h0"]})
+    assert np.array_equal(to_f64_numpy(h[:, :4096]), href)
+
+
+def test_affine_running_product_and_geometric(cuda_device):
+    """u≡0 gives h0*prod(a) (a=0.5: exact powers of two until underflow); constant a,u gives
+    the geometric series (BJ closed forms), here against the closed form itself."""
+    L = 100
+    inp = {"a": torch.full((1, L), 0.5, device=cuda_device), "u": torch.zeros((1, L), device=cuda_device),
+           "h0": torch.tensor([3.0], device=cuda_device)}
+    for v in AFFINE_VARIANTS:
+        h, _ = gpu_affine(inp, v)
+        assert np.array_equal(to_f64_numpy(h[0]), np.ldexp(3.0, -np.arange(1, L + 1)))
+    L = 5000
+    a0, u0, h00 = 0.999, 0.01, -1.0
+    inp = {"a": torch.full((1, L), a0, device=cuda_device), "u": torch.full((1, L), u0, device=cuda_device),
+           "h0": torch.tensor([h00], device=cuda_device)}
+    a0f, u0f = float(np.float32(a0)), float(np.float32(u0))
+    t1 = np.arange(1, L + 1, dtype=np.float64)
+    ref = a0f ** t1 * h00 + u0f * (1 - a0f ** t1) / (1 - a0f)
+    for v in AFFINE_VARIANTS:
+        h, _ = gpu_affine(inp, v)
+        assert_close(h[0], ref, torch.float32, f"geometric v={v}")
+
+
+def test_affine_optional_outputs_and_empty(cuda_device):
+    inp = _affine_inputs(4, 1000, torch.float32, cuda_device, 11, with_h0=False)
+    h1, _ = gpu_affine(inp, want_h_last=False)
+    h2, hl = gpu_affine(inp)
+    assert torch.equal(h1, h2) and torch.equal(hl, h2[:, -1])
+    # L == 0: h_last <- h0 (or 0); num_seq == 0: no-op
+    h0 = torch.tensor([1.5, -2.5], device=cuda_device)
+    e = torch.empty((2, 0), device=cuda_device)
+    hl = torch.full((2,), float("nan"), device=cuda_device)
+    lib.affine_scan(e, e, h0, torch.empty_like(e), hl)
+    torch.cuda.synchronize()
+    assert torch.equal(hl, h0)
+    lib.affine_scan(e, e, None, torch.empty_like(e), hl)
+    torch.cuda.synchronize()
+    assert torch.equal(hl, torch.zeros_like(hl))
+    z = torch.empty((0, 8), device=cuda_device)
+    lib.affine_scan(z, z, None, torch.empty_like(z), None)
+
+
+def test_affine_misaligned_pointers_take_the_scalar_path(cuda_device):
+    """Views offset by one element break 16-byte alignment: not an error (header)."""
+    S, L = 3, 1000
+    for dtype in DTYPES:
+        base = _affine_inputs(1, S * L + 1, dtype, cuda_device, 31, with_h0=False)
+        a = base["a"].reshape(-1)[1:].reshape(S, L)
+        u = base["u"].reshape(-1)[1:].reshape(S, L)
+        assert a.data_ptr() % 16 != 0 and a.is_contiguous()
+        inp = {"a": a, "u": u, "h0": None}
+        for v in AFFINE_VARIANTS:
+            hbuf = torch.empty(S * L + 1, dtype=dtype, device=cuda_device)
+            h = hbuf[1:].reshape(S, L)
+            hl = torch.empty(S, device=cuda_device)
+            lib.affine_scan_ex(a, u, None, h, hl, v)
+            torch.cuda.synchronize()
+            href, hlref = oracle_affine(inp)
+            assert_close(h, href, dtype, f"misaligned v={v}")
+            assert_close(hl, hlref, dtype, f"misaligned h_last v={v}")
+
+
+def test_affine_variants_agree_and_are_deterministic(cuda_device):
+    inp = _affine_inputs(7, 50_000, torch.float32, cuda_device, 77)
+    outs = []
+    for v in AFFINE_VARIANTS:
+        h1, hl1 = gpu_affine(inp, v)
+        h2, hl2 = gpu_affine(inp, v)
+        assert torch.equal(h1, h2) and torch.equal(hl1, hl2), f"variant {v} not reproducible"
+        outs.append(h1)
+    for o in outs[1:]:
+        assert rel_err(o, to_f64_numpy(outs[0])) <= 2 * TOL[torch.float32]
+
+
+def test_affine_split_invariance_chains_h_last_into_h0(cuda_device):
+    """Eq.5 / P:93: one call over L equals two chained calls through h_last -> h0."""
+    inp = _affine_inputs(4, 9000, torch.float32, cuda_device, 5)
+    h, hl = gpu_affine(inp)
+    m = 4096 + 8
+    ha, hla = gpu_affine({"a": inp["a"][:, :m].contiguous(), "u": inp["u"][:, :m].contiguous(),
+                          "h0": inp["h0"]})
+    hb, hlb = gpu_affine({"a": inp["a"][:, m:].contiguous(), "u": inp["u"][:, m:].contiguous(),
+                          "h0": hla})
+    ref = to_f64_numpy(h)
+    assert rel_err(torch.cat([ha, hb], dim=1), ref) <= 1e-5
+    assert rel_err(hlb, to_f64_numpy(hl)) <= 1e-5
+
+
+def test_affine_weighted_prefix_recurrence(cuda_device):
+    """P:272 Eq.(10): h_t = alpha_t h_{t-1} + beta_t is affine_scan(a=alpha, u=beta)."""
+    S, L = 3, 3000
+    alpha = uniform((S, L), 0.2, 1.0, seed=9, stream=0, device=cuda_device, dtype=torch.float32)
+    beta = normal((S, L), seed=9, stream=1, device=cuda_device, dtype=torch.float32)
+    check_affine({"a": alpha, "u": beta, "h0": None}, what="weighted prefix")
+
+
+def test_affine_host_api_matches_device_api(cuda_device):
+    inp = _affine_inputs(5, 3000, torch.float32, cuda_device, 13)
+    h, hl = gpu_affine(inp)
+    a, u, h0 = inp["a"].cpu().pin_memory(), inp["u"].cpu().pin_memory(), inp["h0"].cpu()
+    hh = torch.empty_like(a).pin_memory()
+    hhl = torch.empty(5)
+    lib.affine_scan_host(a, u, h0, hh, hhl)
+    assert torch.equal(hh, h.cpu()) and torch.equal(hhl, hl.cpu())
+
+
+# ================================================================ selective: T1 shapes
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_selective_warp_row_small_and_ragged_shapes(cuda_device, dtype):
+    seed = 200
+    for (batch, d_inner, N, L) in [
+        (1, 1, 16, 1), (1, 1, 16, 2), (2, 3, 16, 7), (1, 5, 16, 8), (2, 2, 16, 31), (1, 2, 16, 33),
+        (1, 3, 16, 255), (2, 4, 16, 256), (1, 2, 16, 257), (1, 2, 16, 511), (1, 3, 16, 512),
+        (1, 2, 16, 513), (2, 33, 16, 1024), (1, 31, 16, 1032), (1, 2, 16, 2047), (1, 2, 16, 2056),
+        (1, 3, 1, 300), (1, 3, 4, 300), (2, 2, 33, 264), (1, 2, 64, 520), (1, 2, 17, 100),
+    ]:
+        seed += 1
+        inp = _selective_inputs(batch, d_inner, N, L, dtype, cuda_device, seed,
+                                with_D=(seed % 3 != 0), with_h0=(seed % 2 == 0))
+        check_selective(inp, lib.SELECTIVE_WARP_ROW, f"warp_row {batch}x{d_inner}x{N}x{L} {dtype}")
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_selective_lane_row_small_and_ragged_shapes(cuda_device, dtype):
+    seed = 300
+    vec = 4 if dtype == torch.float32 else 8
+    for (batch, d_inner, L) in [
+        (1, 32, vec), (1, 32, 2 * vec), (2, 32, 64 - vec), (1, 64, 64), (2, 32, 64 + vec),
+        (1, 96, 128), (1, 32, 192 - vec), (3, 160, 200), (1, 128, 1024), (2, 256, 520),
+    ]:
+        seed += 1
+        inp = _selective_inputs(batch, d_inner, 16, L, dtype, cuda_device, seed,
+                                with_D=(seed % 3 != 0), with_h0=(seed % 2 == 0))
+        assert lane_row_ok(inp)
+        check_selective(inp, lib.SELECTIVE_LANE_ROW, f"lane_row {batch}x{d_inner}x{L} {dtype}")
+
+
+def test_selective_forced_lane_row_rejects_unsupported_shapes(cuda_device):
+    inp = _selective_inputs(1, 33, 16, 64, torch.float32, cuda_device, 1)
+    with pytest.raises(lib.AffineScanError) as ei:
+        gpu_selective(inp, lib.SELECTIVE_LANE_ROW)
+    assert ei.value.status == 4
+    inp = _selective_inputs(1, 32, 8, 64, torch.float32, cuda_device, 1)
+    with pytest.raises(lib.AffineScanError):
+        gpu_selective(inp, lib.SELECTIVE_LANE_ROW)
+    with pytest.raises(lib.AffineScanError):
+        gpu_selective(inp, lib.AFFINE_LOOKBACK)      # not a selective variant
+    gpu_selective(inp, lib.VARIANT_AUTO)             # AUTO falls back to warp_row
+    assert lib.last_variant() == lib.SELECTIVE_WARP_ROW
+
+
+def test_selective_variants_agree_and_are_deterministic(cuda_device):
+    inp = _selective_inputs(2, 64, 16, 1536, torch.float32, cuda_device, 21, with_h0=True)
+    y1, hl1 = gpu_selective(inp, lib.SELECTIVE_WARP_ROW)
+    y1b, hl1b = gpu_selective(inp, lib.SELECTIVE_WARP_ROW)
+    y2, hl2 = gpu_selective(inp, lib.SELECTIVE_LANE_ROW)
+    y2b, hl2b = gpu_selective(inp, lib.SELECTIVE_LANE_ROW)
+    assert torch.equal(y1, y1b) and torch.equal(hl1, hl1b)
+    assert torch.equal(y2, y2b) and torch.equal(hl2, hl2b)
+    assert rel_err(y2, to_f64_numpy(y1)) <= 2 * TOL[torch.float32]
+    assert rel_err(hl2, to_f64_numpy(hl1)) <= 2 * TOL[torch.float32]
+
+
+@pytest.mark.parametrize("variant", [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW])
+def test_selective_split_invariance(cuda_device, variant):
+    inp = _selective_inputs(1, 32, 16, 2048, torch.float32, cuda_device, 8, with_h0=True)
+    y, hl = gpu_selective(inp, variant)
+    m = 1000
+    first = {k: (v[..., :m].contiguous() if k in ("x", "delta", "B", "C") else v)
+             for k, v in inp.items()}
+    y1, hl1 = gpu_selective(first, variant)
+    second = {k: (v[..., m:].contiguous() if k in ("x", "delta", "B", "C") else v)
+              for k, v in inp.items()}
+    second["h0"] = hl1
+    y2, hl2 = gpu_selective(second, variant)
+    assert rel_err(torch.cat([y1, y2], dim=2), to_f64_numpy(y)) <= 1e-5
+    assert rel_err(hl2, to_f64_numpy(hl)) <= 1e-5
+
+
+@pytest.mark.parametrize("variant", [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW])
+def test_selective_degenerate_cases(cuda_device, variant):
+    """delta≡0 holds the state (y = C·h0 + D·x); N=1-like reduction with one-hot C."""
+    dev = cuda_device
+    inp = _selective_inputs(1, 32, 16, 256, torch.float32, dev, 4, with_h0=True)
+    inp["delta"] = torch.zeros_like(inp["delta"])
+    y, hl = gpu_selective(inp, variant)
+    ref = torch.einsum("bnl,bdn->bdl", inp["C"].double(), inp["h0"].double()) \
+        + inp["D"].double()[None, :, None] * inp["x"].double()
+    assert rel_err(y, ref.cpu().numpy()) <= 1e-5
+    assert torch.equal(hl, inp["h0"])
+    # one-hot C picks state n: y equals the affine scan of (exp(ΔA_n), ΔB_n x), via the oracle
+    inp = _selective_inputs(1, 32, 16, 256, torch.float32, dev, 5, with_D=False)
+    n = 5
+    C = torch.zeros_like(inp["C"])
+    C[:, n, :] = 1.0
+    inp["C"] = C
+    y, _ = gpu_selective(inp, variant)
+    a = np.exp(to_f64_numpy(inp["delta"])[0] * to_f64_numpy(inp["A"])[:, n:n + 1])
+    u = to_f64_numpy(inp["delta"])[0] * to_f64_numpy(inp["B"])[0, n][None, :] * to_f64_numpy(inp["x"])[0]
+    href, _ = oracle.affine_scan(a, u, None)
+    assert_close(y[0], href, torch.float32, "one-hot C")
+
+
+def test_selective_optional_outputs_and_empty(cuda_device):
+    inp = _selective_inputs(1, 32, 16, 128, torch.float32, cuda_device, 6)
+    for v in (lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW):
+        y1, _ = gpu_selective(inp, v, want_h_last=False)
+        y2, _ = gpu_selective(inp, v)
+        assert torch.equal(y1, y2)
+    # L == 0
+    e = torch.empty((1, 32, 0), device=cuda_device)
+    bc = torch.empty((1, 16, 0), device=cuda_device)
+    h0 = normal((1, 32, 16), seed=1, stream=0, device=cuda_device, dtype=torch.float32)
+    hl = torch.full_like(h0, float("nan"))
+    lib.selective_scan_fwd(e, e, inp["A"], bc, bc, None, h0, torch.empty_like(e), hl)
+    torch.cuda.synchronize()
+    assert torch.equal(hl, h0)
+
+
+def test_selective_host_api_matches_device_api(cuda_device):
+    inp = _selective_inputs(2, 64, 16, 512, torch.bfloat16, cuda_device, 17)
+    y, hl = gpu_selective(inp)
+    host = {k: (None if v is None else v.cpu()) for k, v in inp.items()}
+    yh = torch.empty_like(host["x"]).pin_memory()
+    hlh = torch.empty((2, 64, 16))
+    lib.selective_scan_fwd_host(host["x"].pin_memory(), host["delta"].pin_memory(), host["A"],
+                                host["B"], host["C"], host["D"], None, yh, hlh)
+    assert torch.equal(yh, y.cpu()) and torch.equal(hlh, hl.cpu())
+
+
+def test_runs_on_a_non_default_stream_and_counts_launches(cuda_device):
+    inp = _selective_inputs(1, 32, 16, 256, torch.float32, cuda_device, 3)
+    s = torch.cuda.Stream()
+    n0 = lib.launch_count()
+    with torch.cuda.stream(s):
+        y, hl = gpu_selective(inp, stream=s)
+    assert lib.launch_count() == n0 + 1
+    yref, _ = oracle_selective(inp)
+    assert_close(y, yref, torch.float32, "stream")
+
+
+# ======================================================== T2: the five BASELINE configs
+def test_config1_affine_fp32_full(cuda_device):
+    inp = make_affine_inputs(config(1), device=cuda_device)
+    for v in [lib.VARIANT_AUTO] + AFFINE_VARIANTS:
+        check_affine(inp, v, f"cfg1 v={v}")
+    inp2 = make_affine_inputs(config(1, seed_offset=1), device=cuda_device)
+    check_affine(inp2, what="cfg1 seed+1")
+
+
+def test_config2_selective_fp32_full(cuda_device):
+    inp = make_selective_inputs(config(2), device=cuda_device)
+    yref, hlref = oracle_selective(inp)
+    for v in (lib.VARIANT_AUTO, lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW):
+        y, hl = gpu_selective(inp, v)
+        assert_close(y, yref, torch.float32, f"cfg2 y v={v}")
+        assert_close(hl, hlref, torch.float32, f"cfg2 h_last v={v}")
+
+
+def _sample_rows(batch, d_inner, k, seed):
+    rng = np.random.default_rng(seed)
+    rows = {(0, 0), (batch - 1, d_inner - 1), (0, d_inner - 1), (batch - 1, 0)}
+    while len(rows) < k:
+        rows.add((int(rng.integers(batch)), int(rng.integers(d_inner))))
+    return sorted(rows)
+
+
+def _check_selective_sampled(inp, variant, rows, dtype, what):
+    y, hl = gpu_selective(inp, variant)
+    assert torch.isfinite(y.float()).all() and torch.isfinite(hl).all()
+    yref, hlref = oracle_selective_rows(inp, rows)
+    bi = torch.tensor([r[0] for r in rows], device=y.device)
+    di = torch.tensor([r[1] for r in rows], device=y.device)
+    assert_close(y[bi, di], yref, dtype, f"{what} y")
+    assert_close(hl[bi, di], hlref, dtype, f"{what} h_last")
+    return y, hl
+
+
+def test_config3_selective_bf16_mamba_scale_sampled_rows(cuda_device):
+    """Full size, in the launch configuration bench.py times (AUTO), on sampled rows the
+    oracle computes one by one; plus both forced variants."""
+    c = config(3)
+    inp = make_selective_inputs(c, device=cuda_device)
+    rows = _sample_rows(c.batch, c.d_inner, 96, 3)
+    y, hl = _check_selective_sampled(inp, lib.VARIANT_AUTO, rows, c.dtype, "cfg3 auto")
+    assert lib.last_variant() == lib.SELECTIVE_LANE_ROW
+    y2, hl2 = _check_selective_sampled(inp, lib.SELECTIVE_WARP_ROW, rows, c.dtype, "cfg3 warp_row")
+    # the two schedules agree everywhere (not only on the sampled rows) to bf16 rounding
+    assert rel_err(hl2, to_f64_numpy(hl)) <= 1e-4
+    assert (y.float() - y2.float()).abs().max().item() <= 2e-2 * (1 + y.float().abs().max().item())
+
+
+def test_config4_selective_long_sequence_sampled_rows(cuda_device):
+    c = config(4)
+    inp = make_selective_inputs(c, device=cuda_device)
+    rows = _sample_rows(c.batch, c.d_inner, 24, 4)
+    _check_selective_sampled(inp, lib.VARIANT_AUTO, rows, c.dtype, "cfg4 auto")
+    assert lib.last_variant() == lib.SELECTIVE_WARP_ROW
+    _check_selective_sampled(inp, lib.SELECTIVE_LANE_ROW, rows, c.dtype, "cfg4 lane_row")
+
+
+def test_config5_affine_bandwidth_sweep_sampled_sequences(cuda_device):
+    """2^30 elements re-segmented into L = 2^10 .. 2^20.  Sampled sequences against the oracle;
+    every element against the recurrence itself (a property that holds at any size)."""
+    total = 1 << 30
+    flat = make_affine_inputs(config(5, L=total, total=total), device=cuda_device)
+    a_flat, u_flat = flat["a"].reshape(-1), flat["u"].reshape(-1)
+    h0_all = normal((1 << 20,), seed=config(5).seed, stream=3, device=cuda_device,
+                    dtype=torch.float32)
+    h = torch.empty(total, dtype=torch.float32, device=cuda_device)
+    rng = np.random.default_rng(5)
+    for logL in (10, 12, 14, 16, 18, 20):
+        L = 1 << logL
+        S = total // L
+        a, u, h0 = a_flat.view(S, L), u_flat.view(S, L), h0_all[:S]
+        hv = h.view(S, L)
+        hl = torch.empty(S, dtype=torch.float32, device=cuda_device)
+        lib.affine_scan(a, u, h0, hv, hl)
+        torch.cuda.synchronize()
+        assert lib.last_variant() == lib.AFFINE_LOOKBACK
+        # sampled sequences, element by element
+        seqs = sorted({0, S - 1, *[int(v) for v in rng.integers(S, size=8 if L >= 1 << 18 else 32)]})
+        idx = torch.tensor(seqs, device=cuda_device)
+        href, hlref = oracle.affine_scan(to_f64_numpy(a[idx]), to_f64_numpy(u[idx]),
+                                         to_f64_numpy(h0[idx]))
+        assert_close(hv[idx], href, torch.float32, f"cfg5 L=2^{logL} h")
+        assert_close(hl[idx], hlref, torch.float32, f"cfg5 L=2^{logL} h_last")
+        # all elements: h_last is the last column; the recurrence holds step by step
+        assert torch.equal(hl, hv[:, -1])
+        worst = 0.0
+        for s0 in range(0, S, max(1, (1 << 26) // L)):
+            s1 = min(S, s0 + max(1, (1 << 26) // L))
+            hb = hv[s0:s1].double()
+            prev = torch.cat([h0[s0:s1].double()[:, None], hb[:, :-1]], dim=1)
+            res = (hb - (a[s0:s1].double() * prev + u[s0:s1].double())).abs() / (1 + hb.abs())
+            worst = max(worst, res.max().item())
+        assert worst <= 1e-5, f"cfg5 L=2^{logL}: recurrence residual {worst:.2e}"

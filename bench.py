@@ -354,6 +354,7 @@ def run_ours(args):
     t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     launches0 = lib.launch_count()
     barrier()
+    torch.cuda.profiler.start()      # ncu --profile-from-start off sees the timed region only
     with ClockSampler(local) as clocks:
         t_begin.record()
         for i in range(K):
@@ -362,6 +363,7 @@ def run_ours(args):
             ev[i][1].record()
         t_end.record()
         torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
     barrier()
     launches = lib.launch_count() - launches0
     total_ms = max_over_ranks(t_begin.elapsed_time(t_end), device)

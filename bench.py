@@ -327,6 +327,8 @@ def run_ours(args):
     from paper_2606_00601_b200.sharding import max_over_ranks
 
     import paper_2606_00601_b200 as lib
+    lib.set_option(lib.OPT_LANE_ROW_G, args.lane_row_g)
+    lib.set_option(lib.OPT_LANE_ROW_POLY16, args.lane_row_poly16)
     w = Workload(args, device)
     c = w.c
     step_bytes = algorithmic_bytes(c, c.kind == "affine" and c.h0_recipe == "normal")
@@ -389,6 +391,9 @@ def run_ours(args):
                 "kernel_ms_median": round(per_launch_ms[K // 2], 5),
                 "frac_of_nominal_8TBps": round(achieved / NOMINAL_HBM_GBS, 4),
                 "kernel": lib.VARIANT_NAMES.get(chosen, str(chosen))}
+    if args.lane_row_g != -1 or args.lane_row_poly16 != -1:
+        roofline["ablation"] = {"lane_row_g": args.lane_row_g,
+                                "lane_row_poly16": args.lane_row_poly16}
     line = {
         "metric": METRIC, "value": value, "unit": "elements/s", "n_gpus": world, "steps": K,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -456,6 +461,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config 1..5 (default 3)")
     ap.add_argument("--L", type=int, default=0, help="sequence length override (config 5 sweep)")
     ap.add_argument("--variant", type=int, default=0, help="force an affinescan_variant")
+    ap.add_argument("--lane-row-g", type=int, default=-1, help="ablation: lanes per row (1, 2, 4)")
+    ap.add_argument("--lane-row-poly16", type=int, default=-1,
+                    help="ablation: sixteenths of the exps on the fma-pipe polynomial (0, 3..6)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)

@@ -171,6 +171,14 @@ AFFINESCAN_API int affinescan_last_variant(void);
 AFFINESCAN_API int64_t affinescan_launch_count(void);
 /* Library version: major*10000 + minor*100 + patch. */
 AFFINESCAN_API int affinescan_version(void);
+/* Tuning knobs for ablations and sweeps (process-wide; -1 restores the default chosen from
+ * the shape).  Returns AFFINESCAN_ERR_UNSUPPORTED for an unknown key or value. */
+typedef enum affinescan_option {
+    AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lanes per (b,d) row in the lane_row schedule: 1, 2, 4 */
+    AFFINESCAN_OPT_LANE_ROW_POLY16 = 2  /* sixteenths (0, 3..6) of the exponentials evaluated by
+                                           the fma-pipe polynomial instead of MUFU.EX2           */
+} affinescan_option;
+AFFINESCAN_API int affinescan_set_option(int key, int value);
 /* Frees the cached scratch / staging buffers of the current device (synchronises it). */
 AFFINESCAN_API int affinescan_release_cache(void);
 

@@ -10,6 +10,8 @@ from .binding import (  # noqa: F401
     AFFINE_LOOKBACK,
     BF16,
     F32,
+    OPT_LANE_ROW_G,
+    OPT_LANE_ROW_POLY16,
     SELECTIVE_LANE_ROW,
     SELECTIVE_WARP_ROW,
     VARIANT_AUTO,
@@ -28,6 +30,7 @@ from .binding import (  # noqa: F401
     selective_scan_fwd,
     selective_scan_fwd_ex,
     selective_scan_fwd_host,
+    set_option,
     status_string,
     version,
 )

@@ -47,7 +47,11 @@ _SIGNATURES = {
     "affinescan_launch_count": (_i64, []),
     "affinescan_version": (_int, []),
     "affinescan_release_cache": (_int, []),
+    "affinescan_set_option": (_int, [_int, _int]),
 }
+
+OPT_LANE_ROW_G = 1
+OPT_LANE_ROW_POLY16 = 2
 
 
 class AffineScanError(RuntimeError):
@@ -236,3 +240,8 @@ def version() -> int:
 
 def release_cache() -> None:
     _check("affinescan_release_cache", load().affinescan_release_cache())
+
+
+def set_option(key: int, value: int) -> None:
+    """Process-wide tuning knob (ablations / sweeps); -1 restores the default."""
+    _check("affinescan_set_option", load().affinescan_set_option(int(key), int(value)))

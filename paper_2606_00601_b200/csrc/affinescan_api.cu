@@ -216,8 +216,10 @@ int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, flo
 
 // ============================================================== selective_scan dispatch
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
-constexpr int kLaneRowTc = 64;      // lane_row: timesteps per staged B/C tile
-constexpr int kLaneRowWarps = 4;    // lane_row: 128 rows per CTA
+constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
+constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
+constexpr int kLaneRowDefaultG = 2;       // lanes per row
+constexpr int kLaneRowDefaultPoly16 = 0;  // sixteenths of the exps done on the fma pipe
 constexpr int64_t kLaneRowMinRows = 148 * 32 * 4;  // one row per FP32 lane of the machine
 
 template <typename T, int VEC, int NV>
@@ -234,13 +236,19 @@ int launch_warp_row(const T* x, const T* delta, const float* A, const T* B, cons
     return after_launch();
 }
 
-template <typename T>
-int launch_lane_row(const T* x, const T* delta, const float* A, const T* B, const T* C,
-                    const float* D, const float* h0, T* y, float* h_last, int batch, int d_inner,
-                    int64_t L, cudaStream_t stream)
+// Tuning knobs of the lane_row schedule (affinescan_set_option); -1 = choose from the shape.
+std::atomic<int> g_opt_lane_row_g{-1};
+std::atomic<int> g_opt_lane_row_poly16{-1};
+
+template <typename T, int G, int F16>
+int launch_lane_row_inst(const T* x, const T* delta, const float* A, const T* B, const T* C,
+                         const float* D, const float* h0, T* y, float* h_last, int batch,
+                         int d_inner, int64_t L, cudaStream_t stream)
 {
+    // polynomial degree per io dtype: DESIGN.md §7 (tolerance argument)
+    constexpr int kDeg = sizeof(T) == 2 ? 3 : 5;
     using S = LaneRowSmem<T, kLaneRowTc>;
-    auto kern = selective_scan_lane_row_kernel<T, kLaneRowTc, kLaneRowWarps>;
+    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg>;
     constexpr int smem = S::kPerWarp * kLaneRowWarps;
     static std::atomic<unsigned> configured{0};  // bit per device
     int dev = 0;
@@ -250,12 +258,55 @@ int launch_lane_row(const T* x, const T* delta, const float* A, const T* B, cons
         configured.fetch_or(1u << (dev & 31));
     }
     const int64_t rows = static_cast<int64_t>(batch) * d_inner;
-    const int64_t warps = rows / 32;
+    const int64_t warps = rows / (32 / G);
     const int64_t blocks = (warps + kLaneRowWarps - 1) / kLaneRowWarps;
     if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
     kern<<<static_cast<unsigned>(blocks), kLaneRowWarps * 32, smem, stream>>>(
         x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, L);
     return after_launch();
+}
+
+template <typename T, int G>
+int launch_lane_row_g(int poly16, const T* x, const T* delta, const float* A, const T* B,
+                      const T* C, const float* D, const float* h0, T* y, float* h_last, int batch,
+                      int d_inner, int64_t L, cudaStream_t stream)
+{
+#define AS_LANE_ROW_CASE(F)                                                                      \
+    case F:                                                                                      \
+        return launch_lane_row_inst<T, G, F>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, \
+                                             L, stream)
+    switch (poly16) {
+        AS_LANE_ROW_CASE(0);
+        AS_LANE_ROW_CASE(3);
+        AS_LANE_ROW_CASE(4);
+        AS_LANE_ROW_CASE(5);
+        AS_LANE_ROW_CASE(6);
+    default: return AFFINESCAN_ERR_UNSUPPORTED;
+    }
+#undef AS_LANE_ROW_CASE
+}
+
+template <typename T>
+int launch_lane_row(const T* x, const T* delta, const float* A, const T* B, const T* C,
+                    const float* D, const float* h0, T* y, float* h_last, int batch, int d_inner,
+                    int64_t L, cudaStream_t stream)
+{
+    int G = g_opt_lane_row_g.load(std::memory_order_relaxed);
+    int poly16 = g_opt_lane_row_poly16.load(std::memory_order_relaxed);
+    if (G < 0) G = kLaneRowDefaultG;
+    if (poly16 < 0) poly16 = kLaneRowDefaultPoly16;
+    switch (G) {
+    case 1:
+        return launch_lane_row_g<T, 1>(poly16, x, delta, A, B, C, D, h0, y, h_last, batch, d_inner,
+                                       L, stream);
+    case 2:
+        return launch_lane_row_g<T, 2>(poly16, x, delta, A, B, C, D, h0, y, h_last, batch, d_inner,
+                                       L, stream);
+    case 4:
+        return launch_lane_row_g<T, 4>(poly16, x, delta, A, B, C, D, h0, y, h_last, batch, d_inner,
+                                       L, stream);
+    default: return AFFINESCAN_ERR_UNSUPPORTED;
+    }
 }
 
 template <typename T>
@@ -470,6 +521,21 @@ int affinescan_last_cuda_error(void) { return tl_last_cuda_error; }
 int affinescan_last_variant(void) { return tl_last_variant; }
 int64_t affinescan_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 int affinescan_version(void) { return 100; }
+
+int affinescan_set_option(int key, int value)
+{
+    switch (key) {
+    case AFFINESCAN_OPT_LANE_ROW_G:
+        if (value != -1 && value != 1 && value != 2 && value != 4) return AFFINESCAN_ERR_UNSUPPORTED;
+        g_opt_lane_row_g.store(value);
+        return AFFINESCAN_OK;
+    case AFFINESCAN_OPT_LANE_ROW_POLY16:
+        if (value != -1 && value != 0 && (value < 3 || value > 6)) return AFFINESCAN_ERR_UNSUPPORTED;
+        g_opt_lane_row_poly16.store(value);
+        return AFFINESCAN_OK;
+    default: return AFFINESCAN_ERR_UNSUPPORTED;
+    }
+}
 
 int affinescan_release_cache(void)
 {

@@ -1,25 +1,29 @@
 // selective_scan_lane_row.cuh — variant AFFINESCAN_SELECTIVE_LANE_ROW of
-// selective_scan_fwd (include/affinescan.h; BJ north_star; SURVEY §8a A1-A10, App. A "G=1").
+// selective_scan_fwd (include/affinescan.h; BJ north_star).
 //
-// One LANE owns one (b,d) row and walks L sequentially with all N=16 states h[n] and
-// A2[n] = A[d,n]*log2(e) in registers: no shuffle, no rescan, no cross-lane reduction —
-// per state-step exactly 1 MUFU.EX2 + 4 FP32 ops (arg, u, h-update, y-accumulate), the
-// minimum the recurrence needs.  This is the schedule for many-row shapes
-// (cfg3: 32768 rows), where the kernel is bound by the SFU/FP32 pipes, not by HBM.
-//
-// A warp = 32 consecutive d of one batch b, so B_t/C_t are warp-uniform.  Each warp
-// stages its [2][N][TC] B/C tile with TMA bulk copies (cp.async.bulk + mbarrier
-// complete_tx, double-buffered), transposes/widens it once to an fp32 [TC][2][N] tile,
-// and then every state-step reads B/C with broadcast LDS.128 (one request serves 4 n for
-// all 32 lanes).  x/delta come from global memory one 128-bit group ahead (register
-// prefetch); y leaves with one 128-bit store per group.  Warps are autonomous: no CTA
-// barrier anywhere.
+// G lanes share one (b,d) row (G = 1, 2 or 4); each lane keeps NS = 16/G of the row's N = 16
+// states h[n] and A2[n] = A[d,n]*log2(e) in registers, packed two states per 64-bit register
+// pair, and walks L sequentially: no warp scan, no rescan.  Per pair of state-steps the work is
+//     arg  = {delta,delta} * A2pair          FMUL2   (fma-pipe, mul.rn.f32x2)
+//     a    = 2^arg                           2 x MUFU.EX2   -- or, for a compile-time share of the
+//                                            (timestep, pair) slots, a Cody-Waite + minimax
+//                                            polynomial 2^x evaluated with FFMA2 on the fma pipe
+//     u    = {delta*x,delta*x} * Bpair       FMUL2
+//     h    = a*h + u                         FFMA2   (Eq.3 with the pair of P:86 Eq.6)
+//     y   += Cpair*h                         FFMA2   (BJ: y = sum_n C h + D x; h never stored)
+// A warp covers 32/G consecutive d of one batch b, so B_t/C_t are warp-uniform: each warp stages
+// its [2][N][TC] B/C tile with TMA bulk copies (cp.async.bulk + mbarrier complete_tx,
+// double-buffered; SASS UBLKCP), transposes/widens it once to an fp32 [TC][2][N] tile, and every
+// state-step then reads B/C with broadcast LDS.128.  x/delta come from global memory as raw
+// 128-bit words prefetched two groups ahead; y is reduced across the G lanes of the row with a
+// shuffle reduce-scatter and leaves with 128/G-bit stores.  Warps are autonomous: no CTA barrier.
 #pragma once
 
 #include "common.cuh"
 
 namespace affinescan {
 
+// ------------------------------------------------------------------ mbarrier / TMA bulk copy
 __device__ __forceinline__ uint32_t smem_u32(const void* p)
 {
     return static_cast<uint32_t>(__cvta_generic_to_shared(p));
@@ -69,6 +73,96 @@ __device__ __forceinline__ void fence_mbar_init()
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
 }
 
+// ------------------------------------------------------------------ packed fp32x2 arithmetic
+// A "pair" is two fp32 values in one 64-bit register pair; SASS: FFMA2 / FMUL2 / FADD2.
+using pair_t = unsigned long long;
+
+__device__ __forceinline__ pair_t pk(float lo, float hi)
+{
+    pair_t r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk(pair_t v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ pair_t fma2(pair_t a, pair_t b, pair_t c)
+{
+    pair_t d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ pair_t mul2(pair_t a, pair_t b)
+{
+    pair_t d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+// ------------------------------------------------------------------ 2^x on the fma pipe
+// x = i + r, i = round(x), r in [-1/2, 1/2];  2^x = 2^i * p(r),  p(r) = 1 + r*q(r) with q the
+// minimax approximation of (2^r - 1)/r (error measured relative to 2^r - 1, so that a = 2^x close
+// to 1 keeps an accurate 1 - a: DESIGN.md §7).  Valid for |x| <= 126 (the caller clamps delta).
+template <int DEG>
+struct Exp2Coef;
+template <>
+struct Exp2Coef<3> {  // max |p - 2^r| / |2^r - 1| = 4.3e-4
+    static __device__ __forceinline__ float c(int i)
+    {
+        constexpr float k[3] = {6.931782961e-01f, 2.420288622e-01f, 5.550396442e-02f};
+        return k[i];
+    }
+};
+template <>
+struct Exp2Coef<4> {  // 1.5e-5
+    static __device__ __forceinline__ float c(int i)
+    {
+        constexpr float k[4] = {6.931368709e-01f, 2.402325273e-01f, 5.583728850e-02f,
+                                9.618110955e-03f};
+        return k[i];
+    }
+};
+template <>
+struct Exp2Coef<5> {  // 4.3e-7 (then fp32 rounding)
+    static __device__ __forceinline__ float c(int i)
+    {
+        constexpr float k[5] = {6.931471229e-01f, 2.402235121e-01f, 5.550500378e-02f,
+                                9.666245431e-03f, 1.333353925e-03f};
+        return k[i];
+    }
+};
+
+// {2^(d*A2.lo), 2^(d*A2.hi)} for dd = {d,d}: 3 + DEG FFMA2 and two integer adds.
+template <int DEG>
+__device__ __forceinline__ pair_t exp2_poly2(pair_t dd, pair_t A2p)
+{
+    constexpr float kMagic = 12582912.0f;  // 1.5 * 2^23: fma rounds x to the nearest integer
+    const pair_t magic = pk(kMagic, kMagic);
+    const pair_t t = fma2(dd, A2p, magic);                   // bits(t) = 0x4B400000 + i
+    const pair_t ni = fma2(t, pk(-1.0f, -1.0f), magic);      // -i, exact
+    const pair_t r = fma2(dd, A2p, ni);                      // x - i with one rounding
+    pair_t q = pk(Exp2Coef<DEG>::c(DEG - 1), Exp2Coef<DEG>::c(DEG - 1));
+#pragma unroll
+    for (int j = DEG - 2; j >= 0; --j) q = fma2(q, r, pk(Exp2Coef<DEG>::c(j), Exp2Coef<DEG>::c(j)));
+    const pair_t p = fma2(q, r, pk(1.0f, 1.0f));
+    float plo, phi, tlo, thi;
+    upk(p, plo, phi);
+    upk(t, tlo, thi);
+    // 2^i by adding i to the exponent field: (bits(t) << 23) == i << 23 (mod 2^32)
+    const float alo = __uint_as_float(__float_as_uint(plo) + (__float_as_uint(tlo) << 23));
+    const float ahi = __uint_as_float(__float_as_uint(phi) + (__float_as_uint(thi) << 23));
+    return pk(alo, ahi);
+}
+
+// Which (timestep-in-group k, pair p) slots use the polynomial: F16 of every 16 slots, spread
+// evenly (Bresenham), decided at compile time.
+__host__ __device__ constexpr bool lane_row_slot_is_poly(int idx, int F16)
+{
+    return ((idx + 1) * F16) / 16 != (idx * F16) / 16;
+}
+
+// ------------------------------------------------------------------ shared-memory plan
 template <typename T, int TC>
 struct LaneRowSmem {
     static constexpr int N = 16;
@@ -78,7 +172,49 @@ struct LaneRowSmem {
     static constexpr int kPerWarp = 2 * kRawStage + kBcTile + 16;            // + 2 mbarriers
 };
 
-template <typename T, int TC, int WARPS>
+// y elements per lane after the reduce-scatter: io-dtype store of CNT consecutive values.
+template <typename T, int CNT>
+__device__ __forceinline__ void store_y(T* p, const float (&v)[CNT]);
+template <>
+__device__ __forceinline__ void store_y<float, 4>(float* p, const float (&v)[4])
+{
+    __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
+}
+template <>
+__device__ __forceinline__ void store_y<float, 2>(float* p, const float (&v)[2])
+{
+    __stcs(reinterpret_cast<float2*>(p), make_float2(v[0], v[1]));
+}
+template <>
+__device__ __forceinline__ void store_y<float, 1>(float* p, const float (&v)[1])
+{
+    __stcs(p, v[0]);
+}
+template <>
+__device__ __forceinline__ void store_y<__nv_bfloat16, 8>(__nv_bfloat16* p, const float (&v)[8])
+{
+    __stcs(reinterpret_cast<uint4*>(p),
+           make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]),
+                      pack_bf16x2(v[6], v[7])));
+}
+template <>
+__device__ __forceinline__ void store_y<__nv_bfloat16, 4>(__nv_bfloat16* p, const float (&v)[4])
+{
+    __stcs(reinterpret_cast<uint2*>(p),
+           make_uint2(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3])));
+}
+template <>
+__device__ __forceinline__ void store_y<__nv_bfloat16, 2>(__nv_bfloat16* p, const float (&v)[2])
+{
+    __stcs(reinterpret_cast<unsigned*>(p), pack_bf16x2(v[0], v[1]));
+}
+
+// ====================================================================================
+// The kernel.  T = io dtype; G = lanes per row; TC = timesteps per staged B/C tile;
+// WARPS = warps per CTA; F16 = sixteenths of the exponentials done by the polynomial;
+// DEG = its degree.
+// ====================================================================================
+template <typename T, int G, int TC, int WARPS, int F16, int DEG>
 __global__ void __launch_bounds__(WARPS * 32)
 selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                const float* __restrict__ A, const T* __restrict__ B,
@@ -88,17 +224,23 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 {
     using S = LaneRowSmem<T, TC>;
     constexpr int N = S::N;
-    constexpr int VEC = Io<T>::kVec;          // timesteps per 128-bit access
-    constexpr int kChunks = TC / VEC;         // 128-bit chunks per raw row
-    using Acc = Access<T, VEC, true>;
+    constexpr int VEC = Io<T>::kVec;   // timesteps per 128-bit access
+    constexpr int kChunks = TC / VEC;  // 128-bit chunks per raw row
+    constexpr int RW = 32 / G;         // rows per warp
+    constexpr int NS = N / G;          // states per lane
+    constexpr int NP = NS / 2;         // packed pairs per lane
+    constexpr int YC = VEC / G;        // y values per lane after the reduce-scatter
+    static_assert(G == 1 || G == 2 || G == 4, "G");
+    static_assert(NS % 4 == 0 && YC >= 1 && TC % VEC == 0 && (TC / VEC) % 2 == 0, "shape");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
+    const int g = lane % G;  // which NS-slice of the row's states
     const long long rows = static_cast<long long>(batch) * d_inner;
-    const long long row0 = (static_cast<long long>(blockIdx.x) * WARPS + warp) * 32;
+    const long long row0 = (static_cast<long long>(blockIdx.x) * WARPS + warp) * RW;
     if (row0 >= rows) return;  // whole warp exits together; warps never sync with each other
-    const long long row = row0 + lane;
+    const long long row = row0 + lane / G;
     const int b = static_cast<int>(row0 / d_inner);  // d_inner % 32 == 0: uniform over the warp
     const int d = static_cast<int>(row - static_cast<long long>(b) * d_inner);
 
@@ -115,7 +257,7 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     __syncwarp();
 
     const long long ntiles = (L + TC - 1) / TC;
-    // lane r stages raw row r: rows 0..15 = B[b, r, :], rows 16..31 = C[b, r-16, :]
+    // A2 staging: lane r copies raw row r: rows 0..15 = B[b, r, :], rows 16..31 = C[b, r-16, :]
     const T* my_src = (lane < N ? B : C) + (static_cast<long long>(b) * N + (lane & (N - 1))) * L;
     auto issue_tile = [&](long long tile) {
         const int st = static_cast<int>(tile & 1);
@@ -129,27 +271,45 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     issue_tile(0);
     if (ntiles > 1) issue_tile(1);
 
-    // per-row constants and state
-    float A2[N], h[N];
+    // per-row constants and state, packed two states per register pair
+    pair_t A2p[NP], h2[NP];
+    float amax = 0.0f;
 #pragma unroll
-    for (int q = 0; q < N / 4; ++q) {
-        const float4 av = __ldg(reinterpret_cast<const float4*>(A + static_cast<long long>(d) * N) + q);
-        A2[4 * q + 0] = av.x * kLog2e; A2[4 * q + 1] = av.y * kLog2e;
-        A2[4 * q + 2] = av.z * kLog2e; A2[4 * q + 3] = av.w * kLog2e;
+    for (int q = 0; q < NS / 4; ++q) {
+        const float4 av =
+            __ldg(reinterpret_cast<const float4*>(A + static_cast<long long>(d) * N + g * NS) + q);
+        A2p[2 * q + 0] = pk(av.x * kLog2e, av.y * kLog2e);
+        A2p[2 * q + 1] = pk(av.z * kLog2e, av.w * kLog2e);
+        amax = fmaxf(fmaxf(fabsf(av.x), fabsf(av.y)), fmaxf(fmaxf(fabsf(av.z), fabsf(av.w)), amax));
         float4 hv = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (h0) hv = __ldg(reinterpret_cast<const float4*>(h0 + row * N) + q);
-        h[4 * q + 0] = hv.x; h[4 * q + 1] = hv.y; h[4 * q + 2] = hv.z; h[4 * q + 3] = hv.w;
+        if (h0) hv = __ldg(reinterpret_cast<const float4*>(h0 + row * N + g * NS) + q);
+        h2[2 * q + 0] = pk(hv.x, hv.y);
+        h2[2 * q + 1] = pk(hv.z, hv.w);
     }
-    const float Dd = D ? __ldg(D + d) : 0.0f;
+    // the polynomial needs |delta*A2| <= 126: clamp delta (2^-126 vs anything smaller: < 1e-37)
+    const float dmax = 126.0f / (amax * kLog2e);
+    const float Dg = (D && g == 0) ? __ldg(D + d) : 0.0f;  // the skip term is added by one lane
 
     const T* xr = x + row * L;
     const T* dr = delta + row * L;
     T* yr = y + row * L;
+    // timestep offset, inside a VEC group, of the YC values this lane stores
+    int yoff = 0;
+    if (G >= 2) yoff += (g & (G / 2)) ? VEC / 2 : 0;
+    if (G >= 4) yoff += (g & 1) ? VEC / 4 : 0;
 
-    // A1: register prefetch, one 128-bit group (VEC timesteps) ahead
-    float xn[VEC], dn[VEC];
-    Acc::load(xr, xn);
-    Acc::load(dr, dn);
+    // A1: raw 128-bit prefetch, two groups (2*VEC timesteps) ahead
+    constexpr int PD = 2;
+    uint4 xq[PD], dq[PD];
+#pragma unroll
+    for (int i = 0; i < PD; ++i) {
+        xq[i] = make_uint4(0, 0, 0, 0);
+        dq[i] = make_uint4(0, 0, 0, 0);
+        if (static_cast<long long>(i) * VEC < L) {
+            xq[i] = __ldcs(reinterpret_cast<const uint4*>(xr) + i);
+            dq[i] = __ldcs(reinterpret_cast<const uint4*>(dr) + i);
+        }
+    }
 
     for (long long tile = 0; tile < ntiles; ++tile) {
         const int st = static_cast<int>(tile & 1);
@@ -157,9 +317,9 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
         const long long t0 = tile * TC;
         mbar_wait(&full[st], parity);
         __syncwarp();  // every lane is done reading the fp32 tile of the previous iteration
-        // A2: widen + transpose raw [2N][TC] (io dtype) -> bc [TC][2][N] (fp32).
-        // Raw pitch ≡ 16 (mod 128) bytes makes the LDS.128 conflict-free across rows; the
-        // transposed stores hit 32 distinct banks.
+        // A2: widen + transpose raw [2N][TC] (io dtype) -> bc [TC][2][N] (fp32).  Raw pitch
+        // ≡ 16 (mod 128) bytes keeps the LDS.128 conflict-free; the transposed stores hit 32
+        // distinct banks.
 #pragma unroll
         for (int c = 0; c < kChunks; ++c) {
             float v[VEC];
@@ -174,48 +334,98 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
             issue_tile(tile + 2);
         }
 
-        // A3..A9: sequential in t, all N states in registers
-        for (int g = 0; g < kChunks; ++g) {
-            const long long tg = t0 + g * VEC;
-            if (tg >= L) break;  // warp-uniform
-            float xv[VEC], dl[VEC];
+        // A3..A9: sequential in t
+#pragma unroll 1
+        for (int gi = 0; gi < kChunks; gi += PD) {
 #pragma unroll
-            for (int k = 0; k < VEC; ++k) { xv[k] = xn[k]; dl[k] = dn[k]; }
-            if (tg + VEC < L) {
-                Acc::load(xr + tg + VEC, xn);
-                Acc::load(dr + tg + VEC, dn);
-            }
-            float out[VEC];
+            for (int pi = 0; pi < PD; ++pi) {
+                const int grp = gi + pi;
+                const long long tg = t0 + grp * VEC;
+                if (grp < kChunks && tg < L) {  // warp-uniform
+                    float xv[VEC], dl[VEC];
+                    unpack128<T>(xq[pi], xv);
+                    unpack128<T>(dq[pi], dl);
+                    if (tg + PD * VEC < L) {
+                        xq[pi] = __ldcs(reinterpret_cast<const uint4*>(xr + tg + PD * VEC));
+                        dq[pi] = __ldcs(reinterpret_cast<const uint4*>(dr + tg + PD * VEC));
+                    }
+                    float ys[VEC];
 #pragma unroll
-            for (int k = 0; k < VEC; ++k) {
-                const float dlk = dl[k];
-                const float dxk = dlk * xv[k];
-                float acc0 = Dd * xv[k], acc1 = 0.0f;
-                const float4* bc4 = reinterpret_cast<const float4*>(bc + (g * VEC + k) * 2 * N);
+                    for (int k = 0; k < VEC; ++k) {
+                        const float dlk = dl[k];
+                        const float dxk = dlk * xv[k];
+                        const pair_t dd = pk(dlk, dlk);
+                        const pair_t dxx = pk(dxk, dxk);
+                        pair_t ddc = dd;
+                        if (F16 > 0) {
+                            const float dc = fminf(dlk, dmax);
+                            ddc = pk(dc, dc);
+                        }
+                        pair_t y2 = pk(0.0f, 0.0f);
+                        const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS;
 #pragma unroll
-                for (int q = 0; q < N / 4; ++q) {
-                    const float4 b4 = bc4[q];
-                    const float4 c4 = bc4[N / 4 + q];
-                    h[4 * q + 0] = fmaf(ex2_approx(dlk * A2[4 * q + 0]), h[4 * q + 0], dxk * b4.x);
-                    acc0 = fmaf(c4.x, h[4 * q + 0], acc0);
-                    h[4 * q + 1] = fmaf(ex2_approx(dlk * A2[4 * q + 1]), h[4 * q + 1], dxk * b4.y);
-                    acc1 = fmaf(c4.y, h[4 * q + 1], acc1);
-                    h[4 * q + 2] = fmaf(ex2_approx(dlk * A2[4 * q + 2]), h[4 * q + 2], dxk * b4.z);
-                    acc0 = fmaf(c4.z, h[4 * q + 2], acc0);
-                    h[4 * q + 3] = fmaf(ex2_approx(dlk * A2[4 * q + 3]), h[4 * q + 3], dxk * b4.w);
-                    acc1 = fmaf(c4.w, h[4 * q + 3], acc1);
+                        for (int q = 0; q < NS / 4; ++q) {
+                            const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 4 * q);
+                            const ulonglong2 c4 =
+                                *reinterpret_cast<const ulonglong2*>(bct + N + 4 * q);
+#pragma unroll
+                            for (int s = 0; s < 2; ++s) {
+                                const int p = 2 * q + s;
+                                const pair_t Bp = s ? b4.y : b4.x;
+                                const pair_t Cp = s ? c4.y : c4.x;
+                                pair_t a2;
+                                if (lane_row_slot_is_poly(k * NP + p, F16)) {
+                                    a2 = exp2_poly2<DEG>(ddc, A2p[p]);
+                                } else {
+                                    float lo, hi;
+                                    upk(mul2(dd, A2p[p]), lo, hi);
+                                    a2 = pk(ex2_approx(lo), ex2_approx(hi));
+                                }
+                                h2[p] = fma2(a2, h2[p], mul2(dxx, Bp));
+                                y2 = fma2(Cp, h2[p], y2);
+                            }
+                        }
+                        float ylo, yhi;
+                        upk(y2, ylo, yhi);
+                        ys[k] = fmaf(Dg, xv[k], ylo + yhi);
+                    }
+                    // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
+                    // each lane ends with YC fully reduced timesteps) and store
+                    if (G >= 2) {
+                        const bool up = (g & (G / 2)) != 0;
+#pragma unroll
+                        for (int j = 0; j < VEC / 2; ++j) {
+                            const float mine = up ? ys[VEC / 2 + j] : ys[j];
+                            const float send = up ? ys[j] : ys[VEC / 2 + j];
+                            ys[j] = mine + __shfl_xor_sync(kFullMask, send, G / 2);
+                        }
+                    }
+                    if (G >= 4) {
+                        const bool up = (g & 1) != 0;
+#pragma unroll
+                        for (int j = 0; j < VEC / 4; ++j) {
+                            const float mine = up ? ys[VEC / 4 + j] : ys[j];
+                            const float send = up ? ys[j] : ys[VEC / 4 + j];
+                            ys[j] = mine + __shfl_xor_sync(kFullMask, send, 1);
+                        }
+                    }
+                    float out[YC];
+#pragma unroll
+                    for (int j = 0; j < YC; ++j) out[j] = ys[j];
+                    store_y<T, YC>(yr + tg + yoff, out);
                 }
-                out[k] = acc0 + acc1;
             }
-            Acc::store(yr + tg, out);
         }
     }
     // A10: final state
     if (h_last) {
 #pragma unroll
-        for (int q = 0; q < N / 4; ++q)
-            reinterpret_cast<float4*>(h_last + row * N)[q] =
-                make_float4(h[4 * q + 0], h[4 * q + 1], h[4 * q + 2], h[4 * q + 3]);
+        for (int q = 0; q < NS / 4; ++q) {
+            float a0, a1, a2, a3;
+            upk(h2[2 * q + 0], a0, a1);
+            upk(h2[2 * q + 1], a2, a3);
+            reinterpret_cast<float4*>(h_last + row * N + g * NS)[q] = make_float4(a0, a1, a2, a3);
+        }
     }
 }
 

@@ -240,6 +240,45 @@ int launch_warp_row(const T* x, const T* delta, const float* A, const T* B, cons
 std::atomic<int> g_opt_lane_row_g{-1};
 std::atomic<int> g_opt_lane_row_poly16{-1};
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_tiled(EncodeTiledFn* out)
+{
+    static std::atomic<void*> cached{nullptr};
+    void* fn = cached.load(std::memory_order_acquire);
+    if (!fn) {
+        cudaDriverEntryPointQueryResult qres;
+        AS_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !fn) return cuda_fail(cudaErrorNotSupported);
+        cached.store(fn, std::memory_order_release);
+    }
+    *out = reinterpret_cast<EncodeTiledFn>(fn);
+    return AFFINESCAN_OK;
+}
+
+// Tensor map over a [batch*N, L] io-dtype matrix (B or C), box = {box_t timesteps, N rows}.
+template <typename T>
+int make_bc_tensor_map(CUtensorMap* map, const T* base, int64_t rows, int64_t L, int box_t, int N)
+{
+    EncodeTiledFn encode = nullptr;
+    const int st = get_encode_tiled(&encode);
+    if (st != AFFINESCAN_OK) return st;
+    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(L), static_cast<cuuint64_t>(rows)};
+    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(L) * sizeof(T)};
+    const cuuint32_t box[2] = {static_cast<cuuint32_t>(box_t), static_cast<cuuint32_t>(N)};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(map, sizeof(T) == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                                  : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                              2, const_cast<T*>(base), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? AFFINESCAN_OK : cuda_fail(cudaErrorInvalidValue);
+}
+
 template <typename T, int G, int F16>
 int launch_lane_row_inst(const T* x, const T* delta, const float* A, const T* B, const T* C,
                          const float* D, const float* h0, T* y, float* h_last, int batch,
@@ -257,12 +296,17 @@ int launch_lane_row_inst(const T* x, const T* delta, const float* A, const T* B,
         AS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         configured.fetch_or(1u << (dev & 31));
     }
+    CUtensorMap mapB, mapC;
+    int st = make_bc_tensor_map<T>(&mapB, B, static_cast<int64_t>(batch) * 16, L, kLaneRowTc, 16);
+    if (st != AFFINESCAN_OK) return st;
+    st = make_bc_tensor_map<T>(&mapC, C, static_cast<int64_t>(batch) * 16, L, kLaneRowTc, 16);
+    if (st != AFFINESCAN_OK) return st;
     const int64_t rows = static_cast<int64_t>(batch) * d_inner;
     const int64_t warps = rows / (32 / G);
     const int64_t blocks = (warps + kLaneRowWarps - 1) / kLaneRowWarps;
     if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
     kern<<<static_cast<unsigned>(blocks), kLaneRowWarps * 32, smem, stream>>>(
-        x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, L);
+        x, delta, A, mapB, mapC, D, h0, y, h_last, batch, d_inner, L);
     return after_launch();
 }
 
@@ -323,6 +367,7 @@ int selective_dispatch(const void* x_, const void* delta_, const float* A, const
     const bool vec_ok = (L % kVec == 0) && aligned16(x) && aligned16(delta) && aligned16(B) &&
                         aligned16(C) && aligned16(y);
     const bool lane_ok = vec_ok && N == 16 && (d_inner % 32 == 0) && aligned16(A) &&
+                         L < (1LL << 31) - 4096 &&
                          (!h0 || aligned16(h0)) && (!h_last || aligned16(h_last));
     const int64_t rows = static_cast<int64_t>(batch) * d_inner;
     if (variant == AFFINESCAN_VARIANT_AUTO)

@@ -12,12 +12,16 @@
 //     h    = a*h + u                         FFMA2   (Eq.3 with the pair of P:86 Eq.6)
 //     y   += Cpair*h                         FFMA2   (BJ: y = sum_n C h + D x; h never stored)
 // A warp covers 32/G consecutive d of one batch b, so B_t/C_t are warp-uniform: each warp stages
-// its [2][N][TC] B/C tile with TMA bulk copies (cp.async.bulk + mbarrier complete_tx,
-// double-buffered; SASS UBLKCP), transposes/widens it once to an fp32 [TC][2][N] tile, and every
+// its [2][N][TC] B/C tile with two TMA tensor copies per tile (cp.async.bulk.tensor.2d through
+// tensor maps over [batch*N, L], mbarrier complete_tx, double-buffered; SASS UTMALDG), transposes/widens it once to an fp32 [TC][2][N] tile, and every
 // state-step then reads B/C with broadcast LDS.128.  x/delta come from global memory as raw
 // 128-bit words prefetched two groups ahead; y is reduced across the G lanes of the row with a
 // shuffle reduce-scatter and leaves with 128/G-bit stores.  Warps are autonomous: no CTA barrier.
 #pragma once
+
+#include <type_traits>
+
+#include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime)
 
 #include "common.cuh"
 
@@ -62,6 +66,18 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst_smem, const void* src_gme
     asm volatile(
         "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
         ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+// TMA 2-D tiled copy global -> shared through a tensor map: box {TC timesteps, N rows} at
+// element coordinates (c0 = t, c1 = row); out-of-range elements are zero-filled and still
+// counted in complete_tx (SASS: UTMALDG).
+__device__ __forceinline__ void tma_tile_2d_g2s(void* dst_smem, const CUtensorMap* map, int c0,
+                                                int c1, uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes "
+        "[%0], [%1, {%2, %3}], [%4];"
+        ::"r"(smem_u32(dst_smem)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
         : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_smem()
@@ -166,10 +182,11 @@ __host__ __device__ constexpr bool lane_row_slot_is_poly(int idx, int F16)
 template <typename T, int TC>
 struct LaneRowSmem {
     static constexpr int N = 16;
-    static constexpr int kRawPitch = TC * static_cast<int>(sizeof(T)) + 16;  // bytes; ≡16 mod 128
-    static constexpr int kRawStage = 2 * N * kRawPitch;                      // B rows then C rows
-    static constexpr int kBcTile = TC * 2 * N * 4;                           // fp32 [TC][2][N]
-    static constexpr int kPerWarp = 2 * kRawStage + kBcTile + 16;            // + 2 mbarriers
+    static constexpr int kRawPitch = TC * static_cast<int>(sizeof(T));  // bytes per box row
+    static constexpr int kRawStage = 2 * N * kRawPitch;                 // B box then C box
+    static constexpr int kBcTile = TC * 2 * N * 4;                      // fp32 [TC][2][N]
+    static constexpr int kPerWarp = 2 * kRawStage + kBcTile + 128;      // + 2 mbarriers, padded
+    static_assert(kRawStage % 256 == 0 && kPerWarp % 128 == 0, "TMA destinations: 128 B aligned");
 };
 
 // y elements per lane after the reduce-scatter: io-dtype store of CNT consecutive values.
@@ -217,8 +234,10 @@ __device__ __forceinline__ void store_y<__nv_bfloat16, 2>(__nv_bfloat16* p, cons
 template <typename T, int G, int TC, int WARPS, int F16, int DEG>
 __global__ void __launch_bounds__(WARPS * 32)
 selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
-                               const float* __restrict__ A, const T* __restrict__ B,
-                               const T* __restrict__ C, const float* __restrict__ D,
+                               const float* __restrict__ A,
+                               const __grid_constant__ CUtensorMap mapB,
+                               const __grid_constant__ CUtensorMap mapC,
+                               const float* __restrict__ D,
                                const float* __restrict__ h0, T* __restrict__ y,
                                float* __restrict__ h_last, int batch, int d_inner, long long L)
 {
@@ -257,16 +276,17 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     __syncwarp();
 
     const long long ntiles = (L + TC - 1) / TC;
-    // A2 staging: lane r copies raw row r: rows 0..15 = B[b, r, :], rows 16..31 = C[b, r-16, :]
-    const T* my_src = (lane < N ? B : C) + (static_cast<long long>(b) * N + (lane & (N - 1))) * L;
+    // A2 staging: one elected lane issues two tensor copies per tile: box {TC, N} of B[b] and
+    // of C[b] (tensor maps over [batch*N, L]); the tail tile is zero-filled by the TMA unit.
     auto issue_tile = [&](long long tile) {
-        const int st = static_cast<int>(tile & 1);
-        const long long t0 = tile * TC;
-        const long long rem = L - t0;
-        const unsigned row_bytes = static_cast<unsigned>((rem < TC ? rem : TC) * sizeof(T));
-        if (lane == 0) mbar_arrive_expect_tx(&full[st], row_bytes * 2u * N);
-        __syncwarp();
-        tma_bulk_g2s(wbase + st * S::kRawStage + lane * S::kRawPitch, my_src + t0, row_bytes, &full[st]);
+        if (lane == 0) {
+            const int st = static_cast<int>(tile & 1);
+            const int t0 = static_cast<int>(tile * TC);
+            unsigned char* dst = wbase + st * S::kRawStage;
+            mbar_arrive_expect_tx(&full[st], static_cast<unsigned>(S::kRawStage));
+            tma_tile_2d_g2s(dst, &mapB, t0, b * N, &full[st]);
+            tma_tile_2d_g2s(dst + N * S::kRawPitch, &mapC, t0, b * N, &full[st]);
+        }
     };
     issue_tile(0);
     if (ntiles > 1) issue_tile(1);
@@ -286,7 +306,7 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
         h2[2 * q + 0] = pk(hv.x, hv.y);
         h2[2 * q + 1] = pk(hv.z, hv.w);
     }
-    // the polynomial needs |delta*A2| <= 126: clamp delta (2^-126 vs anything smaller: < 1e-37)
+    // the polynomial is used only while |delta*A2| <= 126 for every state of the lane
     const float dmax = 126.0f / (amax * kLog2e);
     const float Dg = (D && g == 0) ? __ldg(D + d) : 0.0f;  // the skip term is added by one lane
 
@@ -317,9 +337,8 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
         const long long t0 = tile * TC;
         mbar_wait(&full[st], parity);
         __syncwarp();  // every lane is done reading the fp32 tile of the previous iteration
-        // A2: widen + transpose raw [2N][TC] (io dtype) -> bc [TC][2][N] (fp32).  Raw pitch
-        // ≡ 16 (mod 128) bytes keeps the LDS.128 conflict-free; the transposed stores hit 32
-        // distinct banks.
+        // A2: widen + transpose raw [2N][TC] (io dtype) -> bc [TC][2][N] (fp32); the
+        // transposed stores hit 32 distinct banks.
 #pragma unroll
         for (int c = 0; c < kChunks; ++c) {
             float v[VEC];
@@ -350,17 +369,14 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         dq[pi] = __ldcs(reinterpret_cast<const uint4*>(dr + tg + PD * VEC));
                     }
                     float ys[VEC];
-#pragma unroll
-                    for (int k = 0; k < VEC; ++k) {
+                    // one timestep for all of this lane's states; F = sixteenths of the exps
+                    // taken by the polynomial (0 on the guarded slow path)
+                    auto step = [&](int k, auto ftag) {
+                        constexpr int F = decltype(ftag)::value;
                         const float dlk = dl[k];
                         const float dxk = dlk * xv[k];
                         const pair_t dd = pk(dlk, dlk);
                         const pair_t dxx = pk(dxk, dxk);
-                        pair_t ddc = dd;
-                        if (F16 > 0) {
-                            const float dc = fminf(dlk, dmax);
-                            ddc = pk(dc, dc);
-                        }
                         pair_t y2 = pk(0.0f, 0.0f);
                         const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS;
 #pragma unroll
@@ -374,8 +390,8 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                                 const pair_t Bp = s ? b4.y : b4.x;
                                 const pair_t Cp = s ? c4.y : c4.x;
                                 pair_t a2;
-                                if (lane_row_slot_is_poly(k * NP + p, F16)) {
-                                    a2 = exp2_poly2<DEG>(ddc, A2p[p]);
+                                if (lane_row_slot_is_poly(k * NP + p, F)) {
+                                    a2 = exp2_poly2<DEG>(dd, A2p[p]);
                                 } else {
                                     float lo, hi;
                                     upk(mul2(dd, A2p[p]), lo, hi);
@@ -388,6 +404,23 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         float ylo, yhi;
                         upk(y2, ylo, yhi);
                         ys[k] = fmaf(Dg, xv[k], ylo + yhi);
+                    };
+                    // the polynomial needs |delta*A2| <= 126; a group in which any lane of the
+                    // warp exceeds that (a underflows: far outside BJ's distributions) takes the
+                    // all-MUFU path instead, so nothing is ever clamped
+                    bool poly_ok = true;
+                    if (F16 > 0) {
+                        float dm = fabsf(dl[0]);
+#pragma unroll
+                        for (int k = 1; k < VEC; ++k) dm = fmaxf(dm, fabsf(dl[k]));
+                        poly_ok = !__any_sync(kFullMask, !(dm <= dmax));
+                    }
+                    if (poly_ok) {
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) step(k, std::integral_constant<int, F16>{});
+                    } else {
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) step(k, std::integral_constant<int, 0>{});
                     }
                     // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
                     // each lane ends with YC fully reduced timesteps) and store

@@ -218,8 +218,8 @@ int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, flo
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
 constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
 constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
-constexpr int kLaneRowDefaultG = 2;       // lanes per row
-constexpr int kLaneRowDefaultPoly16 = 0;  // sixteenths of the exps done on the fma pipe
+constexpr int kLaneRowDefaultG = 1;       // lanes per row (r01b sweep: profiles/)
+constexpr int kLaneRowDefaultPoly16 = 4;  // sixteenths of the exps done on the fma pipe
 constexpr int64_t kLaneRowMinRows = 148 * 32 * 4;  // one row per FP32 lane of the machine
 
 template <typename T, int VEC, int NV>

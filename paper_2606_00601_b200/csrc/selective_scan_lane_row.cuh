@@ -369,41 +369,47 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         dq[pi] = __ldcs(reinterpret_cast<const uint4*>(dr + tg + PD * VEC));
                     }
                     float ys[VEC];
-                    // one timestep for all of this lane's states; F = sixteenths of the exps
-                    // taken by the polynomial (0 on the guarded slow path)
-                    auto step = [&](int k, auto ftag) {
-                        constexpr int F = decltype(ftag)::value;
-                        const float dlk = dl[k];
-                        const float dxk = dlk * xv[k];
-                        const pair_t dd = pk(dlk, dlk);
-                        const pair_t dxx = pk(dxk, dxk);
-                        pair_t y2 = pk(0.0f, 0.0f);
-                        const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS;
+                    // One pass = four states (two packed pairs, one LDS.128 of B and of C per
+                    // timestep) over the VEC timesteps of the group: first every 2^x of the pass
+                    // (independent: they stream through the MUFU / fma pipes back to back), then
+                    // the two dependent h chains.  F = sixteenths of the exps taken by the
+                    // polynomial (0 on the guarded slow path).
+                    float dxs[VEC];
+                    pair_t y2[VEC];
 #pragma unroll
-                        for (int q = 0; q < NS / 4; ++q) {
-                            const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 4 * q);
-                            const ulonglong2 c4 =
-                                *reinterpret_cast<const ulonglong2*>(bct + N + 4 * q);
+                    for (int k = 0; k < VEC; ++k) {
+                        dxs[k] = dl[k] * xv[k];
+                        y2[k] = pk(Dg * xv[k], 0.0f);
+                    }
+                    auto pass = [&](int q, auto ftag) {
+                        constexpr int F = decltype(ftag)::value;
+                        pair_t av[VEC][2];
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            const pair_t dd = pk(dl[k], dl[k]);
 #pragma unroll
                             for (int s = 0; s < 2; ++s) {
                                 const int p = 2 * q + s;
-                                const pair_t Bp = s ? b4.y : b4.x;
-                                const pair_t Cp = s ? c4.y : c4.x;
-                                pair_t a2;
                                 if (lane_row_slot_is_poly(k * NP + p, F)) {
-                                    a2 = exp2_poly2<DEG>(dd, A2p[p]);
+                                    av[k][s] = exp2_poly2<DEG>(dd, A2p[p]);
                                 } else {
                                     float lo, hi;
                                     upk(mul2(dd, A2p[p]), lo, hi);
-                                    a2 = pk(ex2_approx(lo), ex2_approx(hi));
+                                    av[k][s] = pk(ex2_approx(lo), ex2_approx(hi));
                                 }
-                                h2[p] = fma2(a2, h2[p], mul2(dxx, Bp));
-                                y2 = fma2(Cp, h2[p], y2);
                             }
                         }
-                        float ylo, yhi;
-                        upk(y2, ylo, yhi);
-                        ys[k] = fmaf(Dg, xv[k], ylo + yhi);
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            const pair_t dxx = pk(dxs[k], dxs[k]);
+                            const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 4 * q;
+                            const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct);
+                            const ulonglong2 c4 = *reinterpret_cast<const ulonglong2*>(bct + N);
+                            h2[2 * q] = fma2(av[k][0], h2[2 * q], mul2(dxx, b4.x));
+                            h2[2 * q + 1] = fma2(av[k][1], h2[2 * q + 1], mul2(dxx, b4.y));
+                            y2[k] = fma2(c4.x, h2[2 * q], y2[k]);
+                            y2[k] = fma2(c4.y, h2[2 * q + 1], y2[k]);
+                        }
                     };
                     // the polynomial needs |delta*A2| <= 126; a group in which any lane of the
                     // warp exceeds that (a underflows: far outside BJ's distributions) takes the
@@ -417,10 +423,16 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                     }
                     if (poly_ok) {
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) step(k, std::integral_constant<int, F16>{});
+                        for (int q = 0; q < NS / 4; ++q) pass(q, std::integral_constant<int, F16>{});
                     } else {
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) step(k, std::integral_constant<int, 0>{});
+                        for (int q = 0; q < NS / 4; ++q) pass(q, std::integral_constant<int, 0>{});
+                    }
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) {
+                        float ylo, yhi;
+                        upk(y2[k], ylo, yhi);
+                        ys[k] = ylo + yhi;
                     }
                     // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
                     // each lane ends with YC fully reduced timesteps) and store

@@ -73,6 +73,8 @@ typedef enum affinescan_variant {
     AFFINESCAN_AFFINE_BLELLOCH = 3, /* ABLATION: the paper's shared-memory Blelloch
                                        upsweep / root init / downsweep / reconstruction
                                        (P:103-107), CTA-loop carry             */
+    AFFINESCAN_AFFINE_WARP_SEQ = 4, /* one warp per sequence (many short sequences), carry in
+                                       a register, no shared memory, no barrier           */
     /* selective_scan_fwd */
     AFFINESCAN_SELECTIVE_WARP_ROW = 11, /* one warp per (b,d) row, lanes own consecutive
                                            chunks of L, warp-shuffle pair scan            */

@@ -8,6 +8,7 @@ from .binding import (  # noqa: F401
     AFFINE_BLELLOCH,
     AFFINE_CTA_LOOP,
     AFFINE_LOOKBACK,
+    AFFINE_WARP_SEQ,
     BF16,
     F32,
     OPT_LANE_ROW_G,

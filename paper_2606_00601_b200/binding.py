@@ -22,11 +22,13 @@ VARIANT_AUTO = 0
 AFFINE_LOOKBACK = 1
 AFFINE_CTA_LOOP = 2
 AFFINE_BLELLOCH = 3
+AFFINE_WARP_SEQ = 4
 SELECTIVE_WARP_ROW = 11
 SELECTIVE_LANE_ROW = 12
 
 VARIANT_NAMES = {
     0: "auto", 1: "affine_lookback", 2: "affine_cta_loop", 3: "affine_blelloch",
+    4: "affine_warp_seq",
     11: "selective_warp_row", 12: "selective_lane_row",
 }
 

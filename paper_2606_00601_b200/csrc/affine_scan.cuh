@@ -310,6 +310,62 @@ affine_scan_cta_loop_kernel(const T* __restrict__ a, const T* __restrict__ u,
 }
 
 // ====================================================================================
+// Variant AFFINESCAN_AFFINE_WARP_SEQ: one WARP per sequence (many short sequences), carry in a
+// register (A7-i), no shared memory and no barrier: warps of a CTA are independent.
+// ====================================================================================
+template <typename T, int VEC, int J, int WARPS>
+__global__ void __launch_bounds__(WARPS * 32)
+affine_scan_warp_seq_kernel(const T* __restrict__ a, const T* __restrict__ u,
+                            const float* __restrict__ h0, T* __restrict__ h,
+                            float* __restrict__ h_last, long long num_seq, long long L)
+{
+    constexpr int kWarpElems = 32 * VEC * J;
+    using Acc = Access<T, VEC, true>;
+    const int lane = threadIdx.x & 31;
+    const long long gwarp = static_cast<long long>(blockIdx.x) * WARPS + (threadIdx.x >> 5);
+    const long long nwarps = static_cast<long long>(gridDim.x) * WARPS;
+
+    for (long long s = gwarp; s < num_seq; s += nwarps) {
+        const T* as = a + s * L;
+        const T* us = u + s * L;
+        T* hs_out = h + s * L;
+        float carry = h0 ? __ldg(h0 + s) : 0.0f;
+        for (long long t0 = 0; t0 < L; t0 += kWarpElems) {
+            TileRegs<VEC, J> r;
+#pragma unroll
+            for (int j = 0; j < J; ++j) {
+                const long long t = t0 + j * 32 * VEC + lane * VEC;
+                if (t < L) {
+                    Acc::load(as + t, r.av[j]);
+                    Acc::load(us + t, r.uv[j]);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) { r.av[j][k] = 1.0f; r.uv[j][k] = 0.0f; }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < J; ++j) row_scan(r, j, lane);
+            float H = carry;
+#pragma unroll
+            for (int j = 0; j < J; ++j) {
+                const long long t = t0 + j * 32 * VEC + lane * VEC;
+                float hv = apply(r.excl[j], H);
+                float out[VEC];
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    hv = fmaf(r.av[j][k], hv, r.uv[j][k]);
+                    out[k] = hv;
+                }
+                if (t < L) Acc::store(hs_out + t, out);
+                H = apply(r.tot[j], H);
+            }
+            carry = H;
+        }
+        if (h_last && lane == 0) h_last[s] = carry;
+    }
+}
+
+// ====================================================================================
 // Variant AFFINESCAN_AFFINE_BLELLOCH (ABLATION): the paper's schedule (P:103-107,
 // P:163-167; Q3/Q4/Q16) on a shared-memory tile of 2*THREADS pairs:
 // upsweep (tree reduction), root <- (1,0), downsweep (prefix propagation), affine-prefix

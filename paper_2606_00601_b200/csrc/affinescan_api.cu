@@ -103,6 +103,9 @@ size_t elt_size(int io_dtype) { return io_dtype == AFFINESCAN_BF16 ? 2 : 4; }
 // ============================================================== affine_scan dispatch
 constexpr int kAffJ = 4;       // 128-bit vectors per thread per tile
 constexpr int kAffWarps = 8;   // 256 threads
+constexpr int64_t kAffWarpSeqMinSeq = 148 * 64;  // >= 64 independent warps per SM
+constexpr int64_t kAffCtaLoopMinSeq = 148 * 4;   // >= 4 CTAs of 8 warps per SM
+constexpr int64_t kAffCtaLoopMinL = 8192;        // at least two CTA tiles per sequence
 
 template <typename T, int VEC>
 int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float* h_last,
@@ -141,6 +144,17 @@ int launch_affine_cta_loop(const T* a, const T* u, const float* h0, T* h, float*
     return after_launch();
 }
 
+template <typename T, int VEC>
+int launch_affine_warp_seq(const T* a, const T* u, const float* h0, T* h, float* h_last,
+                           int64_t num_seq, int64_t L, cudaStream_t stream)
+{
+    const int64_t blocks = (num_seq + kAffWarps - 1) / kAffWarps;
+    const unsigned grid = static_cast<unsigned>(blocks < 0x7fffffffLL ? blocks : 0x7fffffffLL);
+    affine_scan_warp_seq_kernel<T, VEC, kAffJ, kAffWarps>
+        <<<grid, kAffWarps * 32, 0, stream>>>(a, u, h0, h, h_last, num_seq, L);
+    return after_launch();
+}
+
 template <typename T>
 int launch_affine_blelloch(const T* a, const T* u, const float* h0, T* h, float* h_last,
                            int64_t num_seq, int64_t L, cudaStream_t stream)
@@ -159,9 +173,21 @@ int affine_dispatch(const void* a_, const void* u_, const float* h0, void* h_, f
     T* h = static_cast<T*>(h_);
     constexpr int kVec = Io<T>::kVec;
     const bool vec_ok = (L % kVec == 0) && aligned16(a) && aligned16(u) && aligned16(h);
-    if (variant == AFFINESCAN_VARIANT_AUTO) variant = AFFINESCAN_AFFINE_LOOKBACK;
+    // AUTO: enough sequences to fill the machine with independent warps or
+    // CTAs => carry in a register; otherwise split the flattened stream over tiles with the
+    // decoupled look-back carry.
+    if (variant == AFFINESCAN_VARIANT_AUTO) {
+        if (num_seq >= kAffCtaLoopMinSeq && L >= kAffCtaLoopMinL)
+            variant = AFFINESCAN_AFFINE_CTA_LOOP;
+        else if (num_seq >= kAffWarpSeqMinSeq) variant = AFFINESCAN_AFFINE_WARP_SEQ;
+        else variant = AFFINESCAN_AFFINE_LOOKBACK;
+    }
     int st;
     switch (variant) {
+    case AFFINESCAN_AFFINE_WARP_SEQ:
+        st = vec_ok ? launch_affine_warp_seq<T, kVec>(a, u, h0, h, h_last, num_seq, L, stream)
+                    : launch_affine_warp_seq<T, 1>(a, u, h0, h, h_last, num_seq, L, stream);
+        break;
     case AFFINESCAN_AFFINE_LOOKBACK:
         st = vec_ok ? launch_affine_lookback<T, kVec>(a, u, h0, h, h_last, num_seq, L, stream)
                     : launch_affine_lookback<T, 1>(a, u, h0, h, h_last, num_seq, L, stream);

@@ -18,7 +18,8 @@ from util import (TOL, assert_close, check_affine, check_selective, gpu_affine, 
 
 pytestmark = pytest.mark.gpu
 
-AFFINE_VARIANTS = [lib.AFFINE_LOOKBACK, lib.AFFINE_CTA_LOOP, lib.AFFINE_BLELLOCH]
+AFFINE_VARIANTS = [lib.AFFINE_LOOKBACK, lib.AFFINE_CTA_LOOP, lib.AFFINE_BLELLOCH,
+                   lib.AFFINE_WARP_SEQ]
 DTYPES = [torch.float32, torch.bfloat16]
 
 
@@ -425,7 +426,8 @@ def test_config5_affine_bandwidth_sweep_sampled_sequences(cuda_device):
         hl = torch.empty(S, dtype=torch.float32, device=cuda_device)
         lib.affine_scan(a, u, h0, hv, hl)
         torch.cuda.synchronize()
-        assert lib.last_variant() == lib.AFFINE_LOOKBACK
+        # AUTO: long sequences, enough of them => one CTA each; many short ones => one warp each
+        assert lib.last_variant() == (lib.AFFINE_CTA_LOOP if L >= 8192 else lib.AFFINE_WARP_SEQ)
         # sampled sequences, element by element
         seqs = sorted({0, S - 1, *[int(v) for v in rng.integers(S, size=8 if L >= 1 << 18 else 32)]})
         idx = torch.tensor(seqs, device=cuda_device)

@@ -358,6 +358,9 @@ def run_ours(args):
     barrier()
     torch.cuda.profiler.start()      # ncu --profile-from-start off sees the timed region only
     with ClockSampler(local) as clocks:
+        # Keep the GPU busy while the host enqueues the K launches, so that the device never
+        # waits for the host inside the timed region (short kernels: cfg1, cfg2).
+        torch.cuda._sleep(min(int(K * 6e4), int(4e8)))
         t_begin.record()
         for i in range(K):
             ev[i][0].record()

@@ -78,6 +78,10 @@ typedef enum affinescan_variant {
     /* selective_scan_fwd */
     AFFINESCAN_SELECTIVE_WARP_ROW = 11, /* one warp per (b,d) row, lanes own consecutive
                                            chunks of L, warp-shuffle pair scan            */
+    AFFINESCAN_SELECTIVE_WARP_ROW_TMA = 13, /* same schedule; a CTA = R rows of one batch
+                                               sharing B_t/C_t tiles staged in shared memory
+                                               by TMA tensor copies (needs N == 16, 16-byte
+                                               aligned pointers, L a multiple of the vector) */
     AFFINESCAN_SELECTIVE_LANE_ROW = 12  /* one lane per (b,d) row, sequential in L, x/Δ/y
                                            and B/C tiles staged in shared memory by TMA
                                            bulk copies (needs d_inner % 32 == 0)          */

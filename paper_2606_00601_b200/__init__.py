@@ -15,6 +15,7 @@ from .binding import (  # noqa: F401
     OPT_LANE_ROW_POLY16,
     SELECTIVE_LANE_ROW,
     SELECTIVE_WARP_ROW,
+    SELECTIVE_WARP_ROW_TMA,
     VARIANT_AUTO,
     VARIANT_NAMES,
     AffineScanError,

@@ -25,11 +25,13 @@ AFFINE_BLELLOCH = 3
 AFFINE_WARP_SEQ = 4
 SELECTIVE_WARP_ROW = 11
 SELECTIVE_LANE_ROW = 12
+SELECTIVE_WARP_ROW_TMA = 13
 
 VARIANT_NAMES = {
     0: "auto", 1: "affine_lookback", 2: "affine_cta_loop", 3: "affine_blelloch",
     4: "affine_warp_seq",
     11: "selective_warp_row", 12: "selective_lane_row",
+    13: "selective_warp_row_tma",
 }
 
 _vp = ctypes.c_void_p

@@ -14,6 +14,7 @@
 #include "affine_scan.cuh"
 #include "selective_scan_lane_row.cuh"
 #include "selective_scan_warp_row.cuh"
+#include "selective_scan_warp_row_tma.cuh"
 
 namespace {
 
@@ -241,6 +242,9 @@ int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, flo
 }
 
 // ============================================================== selective_scan dispatch
+constexpr int kSmCount = 148;
+constexpr int kWarpRowTmaMaxWarps = 12;   // warp_row_tma: rows per CTA (384 threads, <= 168 regs)
+constexpr int64_t kWarpRowTmaMinL = 1024; // below two warp tiles the plain warp_row is as good
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
 constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
 constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
@@ -380,6 +384,41 @@ int launch_lane_row(const T* x, const T* delta, const float* A, const T* B, cons
 }
 
 template <typename T>
+int launch_warp_row_tma(const T* x, const T* delta, const float* A, const T* B, const T* C,
+                        const float* D, const float* h0, T* y, float* h_last, int batch,
+                        int d_inner, int64_t L, cudaStream_t stream)
+{
+    constexpr int kVec = Io<T>::kVec;
+    constexpr int kNv = 3;  // odd: conflict-free LDS.128 (K = 12 fp32 / 24 bf16 timesteps per lane)
+    using S = WarpRowTmaSmem<T, kNv * kVec>;
+    constexpr int kNu = sizeof(T) == 2 ? 1 : 2;  // K = 24 leaves no registers for a second chain
+    auto kern = selective_scan_warp_row_tma_kernel<T, kVec, kNv, kNu>;
+    static std::atomic<unsigned> configured{0};  // bit per device
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    if (!(configured.load() & (1u << (dev & 31)))) {
+        AS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::kBytes));
+        configured.fetch_or(1u << (dev & 31));
+    }
+    CUtensorMap mapB, mapC;
+    int st = make_bc_tensor_map<T>(&mapB, B, static_cast<int64_t>(batch) * 16, L, S::kBoxT, 16);
+    if (st != AFFINESCAN_OK) return st;
+    st = make_bc_tensor_map<T>(&mapC, C, static_cast<int64_t>(batch) * 16, L, S::kBoxT, 16);
+    if (st != AFFINESCAN_OK) return st;
+    // R rows (warps) of one batch per CTA, sized so that one wave of CTAs covers all rows when
+    // they fit (cfg2/cfg4: 1536 rows -> 140 CTAs of 11 warps on 148 SMs)
+    const int slots = kSmCount / batch > 0 ? kSmCount / batch : 1;
+    int R = (d_inner + slots - 1) / slots;
+    R = R < 1 ? 1 : (R > kWarpRowTmaMaxWarps ? kWarpRowTmaMaxWarps : R);
+    const int ctas_per_batch = (d_inner + R - 1) / R;
+    const int64_t blocks = static_cast<int64_t>(batch) * ctas_per_batch;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    kern<<<static_cast<unsigned>(blocks), R * 32, S::kBytes, stream>>>(
+        x, delta, A, mapB, mapC, D, h0, y, h_last, batch, d_inner, ctas_per_batch, L);
+    return after_launch();
+}
+
+template <typename T>
 int selective_dispatch(const void* x_, const void* delta_, const float* A, const void* B_,
                        const void* C_, const float* D, const float* h0, void* y_, float* h_last,
                        int batch, int d_inner, int N, int64_t L, int variant, cudaStream_t stream)
@@ -392,13 +431,16 @@ int selective_dispatch(const void* x_, const void* delta_, const float* A, const
     constexpr int kVec = Io<T>::kVec;
     const bool vec_ok = (L % kVec == 0) && aligned16(x) && aligned16(delta) && aligned16(B) &&
                         aligned16(C) && aligned16(y);
-    const bool lane_ok = vec_ok && N == 16 && (d_inner % 32 == 0) && aligned16(A) &&
-                         L < (1LL << 31) - 4096 &&
+    const bool lane_ok_common = vec_ok && L < (1LL << 31) - 4096;  // TMA coordinates are int32
+    const bool lane_ok = lane_ok_common && N == 16 && (d_inner % 32 == 0) && aligned16(A) &&
                          (!h0 || aligned16(h0)) && (!h_last || aligned16(h_last));
     const int64_t rows = static_cast<int64_t>(batch) * d_inner;
-    if (variant == AFFINESCAN_VARIANT_AUTO)
-        variant = (lane_ok && rows >= kLaneRowMinRows) ? AFFINESCAN_SELECTIVE_LANE_ROW
-                                                       : AFFINESCAN_SELECTIVE_WARP_ROW;
+    const bool tma_ok = lane_ok_common && N == 16;
+    if (variant == AFFINESCAN_VARIANT_AUTO) {
+        if (lane_ok && rows >= kLaneRowMinRows) variant = AFFINESCAN_SELECTIVE_LANE_ROW;
+        else if (tma_ok && L >= kWarpRowTmaMinL) variant = AFFINESCAN_SELECTIVE_WARP_ROW_TMA;
+        else variant = AFFINESCAN_SELECTIVE_WARP_ROW;
+    }
     int st;
     switch (variant) {
     case AFFINESCAN_SELECTIVE_WARP_ROW:
@@ -408,6 +450,10 @@ int selective_dispatch(const void* x_, const void* delta_, const float* A, const
         else
             st = launch_warp_row<T, 1, 4>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, N, L,
                                           stream);
+        break;
+    case AFFINESCAN_SELECTIVE_WARP_ROW_TMA:
+        if (!tma_ok) return AFFINESCAN_ERR_UNSUPPORTED;
+        st = launch_warp_row_tma<T>(x, delta, A, B, C, D, h0, y, h_last, batch, d_inner, L, stream);
         break;
     case AFFINESCAN_SELECTIVE_LANE_ROW:
         if (!lane_ok) return AFFINESCAN_ERR_UNSUPPORTED;

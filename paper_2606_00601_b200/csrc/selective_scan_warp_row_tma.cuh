@@ -1,0 +1,256 @@
+// selective_scan_warp_row_tma.cuh — variant AFFINESCAN_SELECTIVE_WARP_ROW_TMA of
+// selective_scan_fwd (include/affinescan.h; BJ north_star).
+//
+// The few-rows schedule (cfg2, cfg4: 1536 rows): the scan over L is parallelised inside the
+// warp.  One warp owns one (b,d) row; a warp tile is 32*K consecutive timesteps, lane l owning
+// the K consecutive steps [l*K, l*K+K).  A CTA is R warps = R rows of ONE batch, so B_t/C_t
+// are shared by the whole CTA: an elected thread stages the [N][32*K] tiles of B and of C with
+// TMA tensor copies (cp.async.bulk.tensor.2d, boxes of 256 timesteps x N rows, mbarrier
+// complete_tx) into a 2-stage shared-memory ring; consumers release a stage through an
+// "empty" mbarrier (one arrival per warp).  For each state n (outer loop, NU states per
+// iteration for ILP) a lane
+//   A3  discretises      a_k = ex2(delta_k * A2[n]),  u_k = (delta_k x_k) * B_k[n]   (smem)
+//   A4  composes its K pairs in registers (P via one ex2 of A2[n]*sum(delta))
+//   A5  combines across the warp with a Kogge–Stone __shfl_up_sync pair scan
+//   A7  takes the carry h_in[n] of the previous tile (register, CTA-loop style)
+//   A8  rescans its K steps from the exclusive prefix (a_k, u_k still in registers)
+//   A9  accumulates y_k += C_k[n] * h_k (smem) ; h itself is never stored.
+// x/delta/y move with coalesced 128-bit global accesses (lane owns K contiguous elements).
+#pragma once
+
+#include "selective_scan_lane_row.cuh"  // mbarrier / TMA helpers
+
+namespace affinescan {
+
+template <typename T, int K>
+struct WarpRowTmaSmem {
+    static constexpr int N = 16;
+    static constexpr int kTileT = 32 * K;                    // timesteps per warp tile
+    static constexpr int kBoxT = kTileT / 3;                 // TMA box: <= 256 elements per dim
+    static constexpr int kBoxes = kTileT / kBoxT;            // boxes per tensor per tile
+    static constexpr int kBoxBytes = N * kBoxT * static_cast<int>(sizeof(T));
+    static constexpr int kStageBytes = 2 * kBoxes * kBoxBytes;  // B boxes then C boxes
+    static constexpr int kStages = 2;
+    static constexpr int kBytes = kStages * kStageBytes + 64;   // + full[2], empty[2]
+    static_assert(kTileT % kBoxT == 0 && kBoxT <= 256, "tile is a whole number of boxes");
+    // Bank conflicts: lane l reads the 16-byte chunks l*NV + v (v < NV) of a row.  Box and row
+    // strides are multiples of 128 B, so the 8 lanes of an LDS.128 phase hit distinct 16-byte
+    // slots iff NV is odd (K = 12 for fp32 io, 24 for bf16 io).
+    static_assert((K * sizeof(T) / 16) % 2 == 1, "odd number of 128-bit vectors per lane");
+    static_assert((kBoxT * sizeof(T)) % 128 == 0, "row stride multiple of 128 B");
+};
+
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// NU = states processed together per n-iteration (independent chains for ILP).
+template <typename T, int VEC, int NV, int NU>
+__global__ void __launch_bounds__(384, 1)
+selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict__ delta,
+                                   const float* __restrict__ A,
+                                   const __grid_constant__ CUtensorMap mapB,
+                                   const __grid_constant__ CUtensorMap mapC,
+                                   const float* __restrict__ D, const float* __restrict__ h0,
+                                   T* __restrict__ y, float* __restrict__ h_last, int batch,
+                                   int d_inner, int ctas_per_batch, long long L)
+{
+    constexpr int K = NV * VEC;
+    using S = WarpRowTmaSmem<T, K>;
+    constexpr int N = S::N;
+    using AccS = Access<T, VEC, true>;  // streamed once: x, delta, y
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S::kStages * S::kStageBytes);
+    uint64_t* empty = full + S::kStages;
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int R = blockDim.x >> 5;  // rows (warps) per CTA
+    const int b = blockIdx.x / ctas_per_batch;
+    const int d0 = (blockIdx.x - b * ctas_per_batch) * R;
+    const int d = d0 + warp;
+    const bool active = d < d_inner;  // inactive warps still take part in the stage ring
+    const int dd = active ? d : d_inner - 1;
+    const long long row = static_cast<long long>(b) * d_inner + dd;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < S::kStages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], static_cast<unsigned>(R));
+        }
+        fence_mbar_init();
+    }
+    fence_proxy_async_smem();
+    __syncthreads();
+
+    const long long ntiles = (L + S::kTileT - 1) / S::kTileT;
+    auto issue_tile = [&](long long tile) {  // one thread
+        const int st = static_cast<int>(tile % S::kStages);
+        unsigned char* dst = smem_raw + st * S::kStageBytes;
+        mbar_arrive_expect_tx(&full[st], static_cast<unsigned>(S::kStageBytes));
+#pragma unroll
+        for (int i = 0; i < S::kBoxes; ++i) {
+            const int t0 = static_cast<int>(tile * S::kTileT) + i * S::kBoxT;
+            tma_tile_2d_g2s(dst + i * S::kBoxBytes, &mapB, t0, b * N, &full[st]);
+            tma_tile_2d_g2s(dst + (S::kBoxes + i) * S::kBoxBytes, &mapC, t0, b * N, &full[st]);
+        }
+    };
+    if (threadIdx.x == 0) {
+        issue_tile(0);
+        if (ntiles > 1) issue_tile(1);
+    }
+
+    const T* xr = x + row * L;
+    const T* dr = delta + row * L;
+    T* yr = y + row * L;
+
+    // Lane n keeps A2[n] = A[d,n]*log2(e) and the carry h_in[n]; broadcast by shuffle.
+    float A2r = lane < N ? __ldg(A + static_cast<long long>(dd) * N + lane) * kLog2e : 0.0f;
+    float hcr = (lane < N && h0) ? __ldg(h0 + row * N + lane) : 0.0f;
+    const float Dd = D ? __ldg(D + dd) : 0.0f;
+
+    // byte offset (inside a tensor's stage, state n = 0) of this lane's v-th 128-bit vector
+    int voff[NV];
+#pragma unroll
+    for (int v = 0; v < NV; ++v) {
+        const int t = lane * K + v * VEC;  // timestep inside the tile
+        voff[v] = (t / S::kBoxT) * S::kBoxBytes + (t % S::kBoxT) * static_cast<int>(sizeof(T));
+    }
+
+    // A1: raw 128-bit prefetch of the lane's K timesteps of x and delta, one tile ahead
+    uint4 xq[NV], dq[NV];
+    auto prefetch = [&](long long tile) {
+        const long long tl = tile * S::kTileT + lane * K;
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            xq[v] = make_uint4(0, 0, 0, 0);  // identity padding: delta = 0 => a = 1, u = 0 (Q12)
+            dq[v] = make_uint4(0, 0, 0, 0);
+            if (tl + v * VEC < L) {
+                xq[v] = __ldcs(reinterpret_cast<const uint4*>(xr + tl + v * VEC));
+                dq[v] = __ldcs(reinterpret_cast<const uint4*>(dr + tl + v * VEC));
+            }
+        }
+    };
+    prefetch(0);
+
+    for (long long tile = 0; tile < ntiles; ++tile) {
+        const int st = static_cast<int>(tile % S::kStages);
+        const unsigned parity = static_cast<unsigned>((tile / S::kStages) & 1);
+        const long long tl = tile * S::kTileT + lane * K;  // first timestep of this lane
+        float dl[K], dx[K], yv[K];
+#pragma unroll
+        for (int v = 0; v < NV; ++v) {
+            float xv[VEC], dv[VEC];
+            unpack128<T>(xq[v], xv);
+            unpack128<T>(dq[v], dv);
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) {
+                dl[v * VEC + k] = dv[k];
+                dx[v * VEC + k] = dv[k] * xv[k];
+                yv[v * VEC + k] = Dd * xv[k];
+            }
+        }
+        if (tile + 1 < ntiles) prefetch(tile + 1);
+        float dsum = 0.0f;
+#pragma unroll
+        for (int k = 0; k < K; ++k) dsum += dl[k];
+
+        mbar_wait(&full[st], parity);
+        const unsigned char* sB = smem_raw + st * S::kStageBytes;
+        const unsigned char* sC = sB + S::kBoxes * S::kBoxBytes;
+
+#pragma unroll 1
+        for (int n0 = 0; n0 < N; n0 += NU) {
+            float a[NU][K], u[NU][K];
+            Pair loc[NU];
+            float hin[NU];
+            // ---- A3 + A4 for NU states: independent work, issued back to back
+#pragma unroll
+            for (int j = 0; j < NU; ++j) {
+                const int n = n0 + j;
+                const float A2n = __shfl_sync(kFullMask, A2r, n);
+                hin[j] = __shfl_sync(kFullMask, hcr, n);
+                const unsigned char* bn = sB + n * S::kBoxT * static_cast<int>(sizeof(T));
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    float bv[VEC];
+                    unpack128<T>(*reinterpret_cast<const uint4*>(bn + voff[v]), bv);
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) {
+                        a[j][v * VEC + k] = ex2_approx(dl[v * VEC + k] * A2n);
+                        u[j][v * VEC + k] = dx[v * VEC + k] * bv[k];
+                    }
+                }
+                loc[j] = Pair{ex2_approx(dsum * A2n), u[j][0]};
+            }
+#pragma unroll
+            for (int k = 1; k < K; ++k) {
+#pragma unroll
+                for (int j = 0; j < NU; ++j) loc[j].U = fmaf(a[j][k], loc[j].U, u[j][k]);
+            }
+            // ---- A5: warp combine (NU interleaved Kogge–Stone scans)
+            Pair inc[NU];
+#pragma unroll
+            for (int j = 0; j < NU; ++j) inc[j] = loc[j];
+#pragma unroll
+            for (int dlt = 1; dlt < 32; dlt <<= 1) {
+                Pair pv[NU];
+#pragma unroll
+                for (int j = 0; j < NU; ++j) pv[j] = shfl_up_pair(inc[j], dlt);
+                if (lane >= dlt) {
+#pragma unroll
+                    for (int j = 0; j < NU; ++j) inc[j] = compose(inc[j], pv[j]);
+                }
+            }
+            // ---- A7/A8: carry-in, rescan; A9: y accumulation
+#pragma unroll
+            for (int j = 0; j < NU; ++j) {
+                const int n = n0 + j;
+                Pair ex = shfl_up_pair(inc[j], 1);
+                if (lane == 0) ex = identity_pair();
+                const Pair tot = shfl_pair(inc[j], 31);
+                float hv = apply(ex, hin[j]);
+                const unsigned char* cn = sC + n * S::kBoxT * static_cast<int>(sizeof(T));
+#pragma unroll
+                for (int v = 0; v < NV; ++v) {
+                    float cc[VEC];
+                    unpack128<T>(*reinterpret_cast<const uint4*>(cn + voff[v]), cc);
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) {
+                        hv = fmaf(a[j][v * VEC + k], hv, u[j][v * VEC + k]);
+                        yv[v * VEC + k] = fmaf(cc[k], hv, yv[v * VEC + k]);
+                    }
+                }
+                const float hout = apply(tot, hin[j]);  // state after the tile (uniform)
+                if (lane == n) hcr = hout;
+            }
+        }
+        // release the stage; the producer refills it with tile + 2 once every warp has
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&empty[st]);
+        if (threadIdx.x == 0 && tile + S::kStages < ntiles) {
+            mbar_wait(&empty[st], parity);
+            fence_proxy_async_smem();
+            issue_tile(tile + S::kStages);
+        }
+        // ---- A9: store y
+        if (active) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                if (tl + v * VEC < L) {
+                    float out[VEC];
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) out[k] = yv[v * VEC + k];
+                    AccS::store(yr + tl + v * VEC, out);
+                }
+            }
+        }
+    }
+    // ---- A10: final state
+    if (h_last && active && lane < N) h_last[row * N + lane] = hcr;
+}
+
+}  // namespace affinescan

@@ -200,6 +200,23 @@ def test_selective_warp_row_small_and_ragged_shapes(cuda_device, dtype):
         check_selective(inp, lib.SELECTIVE_WARP_ROW, f"warp_row {batch}x{d_inner}x{N}x{L} {dtype}")
 
 
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_selective_warp_row_tma_small_and_ragged_shapes(cuda_device, dtype):
+    """CTA-shared TMA-staged B/C tiles: one tile, ragged tails, several tiles, rows that do not
+    fill the last CTA, several batches."""
+    seed = 400
+    vec = 4 if dtype == torch.float32 else 8
+    for (batch, d_inner, L) in [
+        (1, 1, vec), (1, 3, 2 * vec), (2, 5, 256), (1, 7, 512 - vec), (1, 2, 512), (2, 3, 512 + vec),
+        (1, 13, 1024), (3, 37, 1536 - vec), (1, 160, 2048), (2, 150, 1000), (1, 1, 4096 + 3 * vec),
+    ]:
+        seed += 1
+        inp = _selective_inputs(batch, d_inner, 16, L, dtype, cuda_device, seed,
+                                with_D=(seed % 3 != 0), with_h0=(seed % 2 == 0))
+        check_selective(inp, lib.SELECTIVE_WARP_ROW_TMA,
+                        f"warp_row_tma {batch}x{d_inner}x{L} {dtype}")
+
+
 @pytest.fixture
 def lane_row_options():
     """Restores the lane_row tuning knobs to their defaults after a test that sets them."""
@@ -270,7 +287,8 @@ def test_selective_variants_agree_and_are_deterministic(cuda_device):
     assert rel_err(hl2, to_f64_numpy(hl1)) <= 2 * TOL[torch.float32]
 
 
-@pytest.mark.parametrize("variant", [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW])
+@pytest.mark.parametrize("variant", [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW,
+                                     lib.SELECTIVE_WARP_ROW_TMA])
 def test_selective_split_invariance(cuda_device, variant):
     inp = _selective_inputs(1, 32, 16, 2048, torch.float32, cuda_device, 8, with_h0=True)
     y, hl = gpu_selective(inp, variant)
@@ -286,7 +304,8 @@ def test_selective_split_invariance(cuda_device, variant):
     assert rel_err(hl2, to_f64_numpy(hl)) <= 1e-5
 
 
-@pytest.mark.parametrize("variant", [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW])
+@pytest.mark.parametrize("variant", [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW,
+                                     lib.SELECTIVE_WARP_ROW_TMA])
 def test_selective_degenerate_cases(cuda_device, variant):
     """delta≡0 holds the state (y = C·h0 + D·x); N=1-like reduction with one-hot C."""
     dev = cuda_device
@@ -360,7 +379,8 @@ def test_config1_affine_fp32_full(cuda_device):
 def test_config2_selective_fp32_full(cuda_device):
     inp = make_selective_inputs(config(2), device=cuda_device)
     yref, hlref = oracle_selective(inp)
-    for v in (lib.VARIANT_AUTO, lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW):
+    for v in (lib.VARIANT_AUTO, lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW,
+              lib.SELECTIVE_WARP_ROW_TMA):
         y, hl = gpu_selective(inp, v)
         assert_close(y, yref, torch.float32, f"cfg2 y v={v}")
         assert_close(hl, hlref, torch.float32, f"cfg2 h_last v={v}")
@@ -395,7 +415,8 @@ def test_config3_selective_bf16_mamba_scale_sampled_rows(cuda_device):
     assert lib.last_variant() == lib.SELECTIVE_LANE_ROW
     y2, hl2 = _check_selective_sampled(inp, lib.SELECTIVE_WARP_ROW, rows, c.dtype, "cfg3 warp_row")
     # the two schedules agree everywhere (not only on the sampled rows) to bf16 rounding
-    assert rel_err(hl2, to_f64_numpy(hl)) <= 1e-4
+    # (lane_row evaluates a share of its 2^x with the degree-3 polynomial for bf16 io: 4.3e-4)
+    assert rel_err(hl2, to_f64_numpy(hl)) <= 2e-3
     assert (y.float() - y2.float()).abs().max().item() <= 2e-2 * (1 + y.float().abs().max().item())
 
 
@@ -404,7 +425,8 @@ def test_config4_selective_long_sequence_sampled_rows(cuda_device):
     inp = make_selective_inputs(c, device=cuda_device)
     rows = _sample_rows(c.batch, c.d_inner, 24, 4)
     _check_selective_sampled(inp, lib.VARIANT_AUTO, rows, c.dtype, "cfg4 auto")
-    assert lib.last_variant() == lib.SELECTIVE_WARP_ROW
+    assert lib.last_variant() == lib.SELECTIVE_WARP_ROW_TMA
+    _check_selective_sampled(inp, lib.SELECTIVE_WARP_ROW, rows, c.dtype, "cfg4 warp_row")
     _check_selective_sampled(inp, lib.SELECTIVE_LANE_ROW, rows, c.dtype, "cfg4 lane_row")
 
 

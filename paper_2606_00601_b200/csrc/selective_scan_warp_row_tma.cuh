@@ -40,6 +40,20 @@ struct WarpRowTmaSmem {
     static_assert((kBoxT * sizeof(T)) % 128 == 0, "row stride multiple of 128 B");
 };
 
+// Non-suspending poll (mbarrier.test_wait) for the short producer-side wait.
+__device__ __forceinline__ void mbar_poll(uint64_t* bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
 __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
@@ -232,7 +246,7 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
         if (threadIdx.x == 0 && tile + S::kStages < ntiles) {
-            mbar_wait(&empty[st], parity);
+            mbar_poll(&empty[st], parity);
             fence_proxy_async_smem();
             issue_tile(tile + S::kStages);
         }

@@ -300,12 +300,15 @@ affine_scan_cta_loop_kernel(const T* __restrict__ a, const T* __restrict__ u,
                     hv = fmaf(r.av[j][k], hv, r.uv[j][k]);
                     out[k] = hv;
                 }
-                if (t < L) Acc::store(hs_out + t, out);
+                if (t < L) {
+                    Acc::store(hs_out + t, out);
+                    // h_last is the very value stored at t = L-1 (bitwise)
+                    if (h_last && t + VEC >= L) h_last[s] = hv;
+                }
                 H = apply(r.tot[j], H);
             }
             carry = apply(agg, carry);
         }
-        if (h_last && threadIdx.x == 0) h_last[s] = carry;
     }
 }
 
@@ -356,12 +359,14 @@ affine_scan_warp_seq_kernel(const T* __restrict__ a, const T* __restrict__ u,
                     hv = fmaf(r.av[j][k], hv, r.uv[j][k]);
                     out[k] = hv;
                 }
-                if (t < L) Acc::store(hs_out + t, out);
+                if (t < L) {
+                    Acc::store(hs_out + t, out);
+                    if (h_last && t + VEC >= L) h_last[s] = hv;  // the value stored at t = L-1
+                }
                 H = apply(r.tot[j], H);
             }
             carry = H;
         }
-        if (h_last && lane == 0) h_last[s] = carry;
     }
 }
 

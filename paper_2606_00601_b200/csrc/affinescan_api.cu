@@ -248,6 +248,7 @@ constexpr int64_t kWarpRowTmaMinL = 1024; // below two warp tiles the plain warp
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
 constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
 constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
+constexpr int kLaneRowPairsPerPass = 2;   // packed pairs per pass (ILP of the MUFU burst)
 constexpr int kLaneRowDefaultG = 1;       // lanes per row (r01b sweep: profiles/)
 constexpr int kLaneRowDefaultPoly16 = 4;  // sixteenths of the exps done on the fma pipe
 constexpr int64_t kLaneRowMinRows = 148 * 32 * 4;  // one row per FP32 lane of the machine
@@ -317,7 +318,9 @@ int launch_lane_row_inst(const T* x, const T* delta, const float* A, const T* B,
     // polynomial degree per io dtype: DESIGN.md §7 (tolerance argument)
     constexpr int kDeg = sizeof(T) == 2 ? 3 : 5;
     using S = LaneRowSmem<T, kLaneRowTc>;
-    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg>;
+    constexpr int kNp = 8 / G;
+    constexpr int kPp = kLaneRowPairsPerPass < kNp ? kLaneRowPairsPerPass : kNp;
+    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg, kPp>;
     constexpr int smem = S::kPerWarp * kLaneRowWarps;
     static std::atomic<unsigned> configured{0};  // bit per device
     int dev = 0;

@@ -229,9 +229,9 @@ __device__ __forceinline__ void store_y<__nv_bfloat16, 2>(__nv_bfloat16* p, cons
 // ====================================================================================
 // The kernel.  T = io dtype; G = lanes per row; TC = timesteps per staged B/C tile;
 // WARPS = warps per CTA; F16 = sixteenths of the exponentials done by the polynomial;
-// DEG = its degree.
+// DEG = its degree; PP = packed pairs per pass (2*PP states share one MUFU burst).
 // ====================================================================================
-template <typename T, int G, int TC, int WARPS, int F16, int DEG>
+template <typename T, int G, int TC, int WARPS, int F16, int DEG, int PP>
 __global__ void __launch_bounds__(WARPS * 32)
 selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                const float* __restrict__ A,
@@ -250,6 +250,7 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     constexpr int NP = NS / 2;         // packed pairs per lane
     constexpr int YC = VEC / G;        // y values per lane after the reduce-scatter
     static_assert(G == 1 || G == 2 || G == 4, "G");
+    static_assert(PP % 2 == 0 && (N / G / 2) % PP == 0, "pairs per pass");
     static_assert(NS % 4 == 0 && YC >= 1 && TC % VEC == 0 && (TC / VEC) % 2 == 0, "shape");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -381,15 +382,15 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         dxs[k] = dl[k] * xv[k];
                         y2[k] = pk(Dg * xv[k], 0.0f);
                     }
-                    auto pass = [&](int q, auto ftag) {
+                    auto pass = [&](int q, auto ftag) {  // pairs [PP*q, PP*q + PP)
                         constexpr int F = decltype(ftag)::value;
-                        pair_t av[VEC][2];
+                        pair_t av[VEC][PP];
 #pragma unroll
                         for (int k = 0; k < VEC; ++k) {
                             const pair_t dd = pk(dl[k], dl[k]);
 #pragma unroll
-                            for (int s = 0; s < 2; ++s) {
-                                const int p = 2 * q + s;
+                            for (int s = 0; s < PP; ++s) {
+                                const int p = PP * q + s;
                                 if (lane_row_slot_is_poly(k * NP + p, F)) {
                                     av[k][s] = exp2_poly2<DEG>(dd, A2p[p]);
                                 } else {
@@ -402,13 +403,19 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 #pragma unroll
                         for (int k = 0; k < VEC; ++k) {
                             const pair_t dxx = pk(dxs[k], dxs[k]);
-                            const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 4 * q;
-                            const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct);
-                            const ulonglong2 c4 = *reinterpret_cast<const ulonglong2*>(bct + N);
-                            h2[2 * q] = fma2(av[k][0], h2[2 * q], mul2(dxx, b4.x));
-                            h2[2 * q + 1] = fma2(av[k][1], h2[2 * q + 1], mul2(dxx, b4.y));
-                            y2[k] = fma2(c4.x, h2[2 * q], y2[k]);
-                            y2[k] = fma2(c4.y, h2[2 * q + 1], y2[k]);
+                            const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 2 * PP * q;
+#pragma unroll
+                            for (int s = 0; s < PP; s += 2) {
+                                const int p = PP * q + s;
+                                const ulonglong2 b4 =
+                                    *reinterpret_cast<const ulonglong2*>(bct + 2 * s);
+                                const ulonglong2 c4 =
+                                    *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
+                                h2[p] = fma2(av[k][s], h2[p], mul2(dxx, b4.x));
+                                h2[p + 1] = fma2(av[k][s + 1], h2[p + 1], mul2(dxx, b4.y));
+                                y2[k] = fma2(c4.x, h2[p], y2[k]);
+                                y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
+                            }
                         }
                     };
                     // the polynomial needs |delta*A2| <= 126; a group in which any lane of the
@@ -423,10 +430,10 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                     }
                     if (poly_ok) {
 #pragma unroll
-                        for (int q = 0; q < NS / 4; ++q) pass(q, std::integral_constant<int, F16>{});
+                        for (int q = 0; q < NP / PP; ++q) pass(q, std::integral_constant<int, F16>{});
                     } else {
 #pragma unroll
-                        for (int q = 0; q < NS / 4; ++q) pass(q, std::integral_constant<int, 0>{});
+                        for (int q = 0; q < NP / PP; ++q) pass(q, std::integral_constant<int, 0>{});
                     }
 #pragma unroll
                     for (int k = 0; k < VEC; ++k) {

@@ -243,7 +243,7 @@ int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, flo
 
 // ============================================================== selective_scan dispatch
 constexpr int kSmCount = 148;
-constexpr int kWarpRowTmaMaxWarps = 12;   // warp_row_tma: rows per CTA (384 threads, <= 168 regs)
+constexpr int kWarpRowTmaMaxWarps = 11;   // warp_row_tma: rows per CTA (+1 producer warp = 384 threads)
 constexpr int64_t kWarpRowTmaMinL = 1024; // below two warp tiles the plain warp_row is as good
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
 constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
@@ -416,7 +416,7 @@ int launch_warp_row_tma(const T* x, const T* delta, const float* A, const T* B, 
     const int ctas_per_batch = (d_inner + R - 1) / R;
     const int64_t blocks = static_cast<int64_t>(batch) * ctas_per_batch;
     if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
-    kern<<<static_cast<unsigned>(blocks), R * 32, S::kBytes, stream>>>(
+    kern<<<static_cast<unsigned>(blocks), (R + 1) * 32, S::kBytes, stream>>>(
         x, delta, A, mapB, mapC, D, h0, y, h_last, batch, d_inner, ctas_per_batch, L);
     return after_launch();
 }

@@ -5,9 +5,9 @@
 // warp.  One warp owns one (b,d) row; a warp tile is 32*K consecutive timesteps, lane l owning
 // the K consecutive steps [l*K, l*K+K).  A CTA is R warps = R rows of ONE batch, so B_t/C_t
 // are shared by the whole CTA: an elected thread stages the [N][32*K] tiles of B and of C with
-// TMA tensor copies (cp.async.bulk.tensor.2d, boxes of 256 timesteps x N rows, mbarrier
-// complete_tx) into a 2-stage shared-memory ring; consumers release a stage through an
-// "empty" mbarrier (one arrival per warp).  For each state n (outer loop, NU states per
+// TMA tensor copies (cp.async.bulk.tensor.2d, boxes of 128/256 timesteps x N rows, mbarrier
+// complete_tx) into a 2-stage shared-memory ring; the elected thread lives in a dedicated
+// producer warp; consumers release a stage through an "empty" mbarrier (one arrival per warp).  For each state n (outer loop, NU states per
 // iteration for ILP) a lane
 //   A3  discretises      a_k = ex2(delta_k * A2[n]),  u_k = (delta_k x_k) * B_k[n]   (smem)
 //   A4  composes its K pairs in registers (P via one ex2 of A2[n]*sum(delta))
@@ -81,7 +81,7 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    const int R = blockDim.x >> 5;  // rows (warps) per CTA
+    const int R = (blockDim.x >> 5) - 1;  // rows (consumer warps) per CTA; warp R is the producer
     const int b = blockIdx.x / ctas_per_batch;
     const int d0 = (blockIdx.x - b * ctas_per_batch) * R;
     const int d = d0 + warp;
@@ -112,9 +112,21 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
             tma_tile_2d_g2s(dst + (S::kBoxes + i) * S::kBoxBytes, &mapC, t0, b * N, &full[st]);
         }
     };
-    if (threadIdx.x == 0) {
-        issue_tile(0);
-        if (ntiles > 1) issue_tile(1);
+    // Producer warp: one elected lane keeps the 2-stage ring full; it refills a stage as soon
+    // as every consumer warp has released it, and never touches the data itself.
+    if (warp == R) {
+        if (lane == 0) {
+            for (long long tile = 0; tile < ntiles; ++tile) {
+                if (tile >= S::kStages) {
+                    const long long prev = tile - S::kStages;  // the tile that used this stage
+                    mbar_poll(&empty[prev % S::kStages],
+                              static_cast<unsigned>((prev / S::kStages) & 1));
+                    fence_proxy_async_smem();
+                }
+                issue_tile(tile);
+            }
+        }
+        return;
     }
 
     const T* xr = x + row * L;
@@ -242,14 +254,9 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
                 if (lane == n) hcr = hout;
             }
         }
-        // release the stage; the producer refills it with tile + 2 once every warp has
+        // release the stage; the producer warp refills it with tile + 2 once every warp has
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
-        if (threadIdx.x == 0 && tile + S::kStages < ntiles) {
-            mbar_poll(&empty[st], parity);
-            fence_proxy_async_smem();
-            issue_tile(tile + S::kStages);
-        }
         // ---- A9: store y
         if (active) {
 #pragma unroll

@@ -249,6 +249,7 @@ constexpr int kSelWarps = 4;        // warp_row: rows per CTA
 constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
 constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
 constexpr int kLaneRowPairsPerPass = 2;   // packed pairs per pass (ILP of the MUFU burst)
+constexpr bool kLaneRowPipelined = false;  // ablation: 2^x of pass q+1 between the chain steps of pass q (0.407 vs 0.348 ms)
 constexpr int kLaneRowDefaultG = 1;       // lanes per row (r01b sweep: profiles/)
 constexpr int kLaneRowDefaultPoly16 = 4;  // sixteenths of the exps done on the fma pipe
 constexpr int64_t kLaneRowMinRows = 148 * 32 * 4;  // one row per FP32 lane of the machine
@@ -320,7 +321,8 @@ int launch_lane_row_inst(const T* x, const T* delta, const float* A, const T* B,
     using S = LaneRowSmem<T, kLaneRowTc>;
     constexpr int kNp = 8 / G;
     constexpr int kPp = kLaneRowPairsPerPass < kNp ? kLaneRowPairsPerPass : kNp;
-    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg, kPp>;
+    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg, kPp,
+                                               kLaneRowPipelined>;
     constexpr int smem = S::kPerWarp * kLaneRowWarps;
     static std::atomic<unsigned> configured{0};  // bit per device
     int dev = 0;

@@ -231,7 +231,7 @@ __device__ __forceinline__ void store_y<__nv_bfloat16, 2>(__nv_bfloat16* p, cons
 // WARPS = warps per CTA; F16 = sixteenths of the exponentials done by the polynomial;
 // DEG = its degree; PP = packed pairs per pass (2*PP states share one MUFU burst).
 // ====================================================================================
-template <typename T, int G, int TC, int WARPS, int F16, int DEG, int PP>
+template <typename T, int G, int TC, int WARPS, int F16, int DEG, int PP, bool PIPE>
 __global__ void __launch_bounds__(WARPS * 32)
 selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                const float* __restrict__ A,
@@ -428,7 +428,58 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         for (int k = 1; k < VEC; ++k) dm = fmaxf(dm, fabsf(dl[k]));
                         poly_ok = !__any_sync(kFullMask, !(dm <= dmax));
                     }
-                    if (poly_ok) {
+                    // Software-pipelined form of the same passes (PIPE): the 2^x of pass q+1 are
+                    // issued timestep by timestep between the chain steps of pass q, so that the
+                    // MUFU works in the shadow of the fma pipe inside ONE warp (an in-order warp
+                    // cannot overlap a MUFU burst with anything else of its own).
+                    auto exps = [&](int q, int k, pair_t (&dst)[PP], auto ftag) {
+                        constexpr int F = decltype(ftag)::value;
+                        const pair_t dd = pk(dl[k], dl[k]);
+#pragma unroll
+                        for (int s = 0; s < PP; ++s) {
+                            const int p = PP * q + s;
+                            if (lane_row_slot_is_poly(k * NP + p, F)) {
+                                dst[s] = exp2_poly2<DEG>(dd, A2p[p]);
+                            } else {
+                                float lo, hi;
+                                upk(mul2(dd, A2p[p]), lo, hi);
+                                dst[s] = pk(ex2_approx(lo), ex2_approx(hi));
+                            }
+                        }
+                    };
+                    auto chain = [&](int q, int k, const pair_t (&av)[PP]) {
+                        const pair_t dxx = pk(dxs[k], dxs[k]);
+                        const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 2 * PP * q;
+#pragma unroll
+                        for (int s = 0; s < PP; s += 2) {
+                            const int p = PP * q + s;
+                            const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 2 * s);
+                            const ulonglong2 c4 =
+                                *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
+                            h2[p] = fma2(av[s], h2[p], mul2(dxx, b4.x));
+                            h2[p + 1] = fma2(av[s + 1], h2[p + 1], mul2(dxx, b4.y));
+                            y2[k] = fma2(c4.x, h2[p], y2[k]);
+                            y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
+                        }
+                    };
+                    auto piped = [&](auto ftag) {
+                        constexpr int NQ = NP / PP;
+                        pair_t av[2][VEC][PP];
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) exps(0, k, av[0][k], ftag);
+#pragma unroll
+                        for (int q = 0; q < NQ; ++q) {
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k) {
+                                if (q + 1 < NQ) exps(q + 1, k, av[(q + 1) & 1][k], ftag);
+                                chain(q, k, av[q & 1][k]);
+                            }
+                        }
+                    };
+                    if (PIPE) {
+                        if (poly_ok) piped(std::integral_constant<int, F16>{});
+                        else piped(std::integral_constant<int, 0>{});
+                    } else if (poly_ok) {
 #pragma unroll
                         for (int q = 0; q < NP / PP; ++q) pass(q, std::integral_constant<int, F16>{});
                     } else {

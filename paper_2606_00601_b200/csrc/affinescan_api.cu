@@ -113,7 +113,9 @@ template <typename T, int VEC>
 int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float* h_last,
                            int64_t num_seq, int64_t L, cudaStream_t stream)
 {
-    constexpr int kTile = kAffWarps * 32 * VEC * kAffLookbackJ;
+    // 4096-element tiles for both io dtypes (64 B of a and of u per thread fit 64 registers)
+    constexpr int kJ = VEC == 8 ? kAffLookbackJ / 2 : kAffLookbackJ;
+    constexpr int kTile = kAffWarps * 32 * VEC * kJ;
     const int64_t total = num_seq * L;
     const int64_t ntiles = (total + kTile - 1) / kTile;
     if (ntiles > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
@@ -124,7 +126,7 @@ int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float*
     AS_CUDA(cudaMemsetAsync(scratch, 0, desc_bytes + 16, stream));
     auto* desc = static_cast<unsigned long long*>(scratch);
     auto* ticket = reinterpret_cast<unsigned*>(static_cast<unsigned char*>(scratch) + desc_bytes);
-    affine_scan_lookback_kernel<T, VEC, kAffLookbackJ, kAffWarps>
+    affine_scan_lookback_kernel<T, VEC, kJ, kAffWarps>
         <<<static_cast<unsigned>(ntiles), kAffWarps * 32, 0, stream>>>(a, u, h0, h, h_last, total, L,
                                                                       desc, ticket);
     return after_launch();

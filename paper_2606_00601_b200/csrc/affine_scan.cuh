@@ -104,7 +104,7 @@ __device__ __forceinline__ void seq_pos(long long q0, long long r0, int off, lon
 // ====================================================================================
 template <typename T, int VEC, int J, int WARPS>
 // 4 CTAs / SM (<= 64 registers): tiles in their load phase cover the ones that look back
-__global__ void __launch_bounds__(WARPS * 32, 4)
+__global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32))
 affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
                             const float* __restrict__ h0, T* __restrict__ h,
                             float* __restrict__ h_last, long long total, long long L,

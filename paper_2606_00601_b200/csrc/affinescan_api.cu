@@ -104,6 +104,8 @@ size_t elt_size(int io_dtype) { return io_dtype == AFFINESCAN_BF16 ? 2 : 4; }
 // ============================================================== affine_scan dispatch
 constexpr int kAffJ = 4;       // 128-bit vectors per thread per tile
 constexpr int kAffWarps = 8;   // 256 threads
+constexpr int kAffLookbackWarps = 8;   // (16 warps = 8192-element tiles measured the same on long L,
+                                       // slower on short L)
 constexpr int kAffLookbackJ = 4;  // look-back tiles of 4096 elements (J = 8: 202 registers, 2.5 TB/s)
 constexpr int64_t kAffWarpSeqMinSeq = 148 * 64;  // >= 64 independent warps per SM
 constexpr int64_t kAffCtaLoopMinSeq = 148 * 4;   // >= 4 CTAs of 8 warps per SM
@@ -115,7 +117,7 @@ int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float*
 {
     // 4096-element tiles for both io dtypes (64 B of a and of u per thread fit 64 registers)
     constexpr int kJ = VEC == 8 ? kAffLookbackJ / 2 : kAffLookbackJ;
-    constexpr int kTile = kAffWarps * 32 * VEC * kJ;
+    constexpr int kTile = kAffLookbackWarps * 32 * VEC * kJ;
     const int64_t total = num_seq * L;
     const int64_t ntiles = (total + kTile - 1) / kTile;
     if (ntiles > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
@@ -126,8 +128,8 @@ int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float*
     AS_CUDA(cudaMemsetAsync(scratch, 0, desc_bytes + 16, stream));
     auto* desc = static_cast<unsigned long long*>(scratch);
     auto* ticket = reinterpret_cast<unsigned*>(static_cast<unsigned char*>(scratch) + desc_bytes);
-    affine_scan_lookback_kernel<T, VEC, kJ, kAffWarps>
-        <<<static_cast<unsigned>(ntiles), kAffWarps * 32, 0, stream>>>(a, u, h0, h, h_last, total, L,
+    affine_scan_lookback_kernel<T, VEC, kJ, kAffLookbackWarps>
+        <<<static_cast<unsigned>(ntiles), kAffLookbackWarps * 32, 0, stream>>>(a, u, h0, h, h_last, total, L,
                                                                       desc, ticket);
     return after_launch();
 }

@@ -400,7 +400,9 @@ int launch_warp_row_tma(const T* x, const T* delta, const float* A, const T* B, 
                         int d_inner, int64_t L, cudaStream_t stream)
 {
     constexpr int kVec = Io<T>::kVec;
-    constexpr int kNv = 3;  // odd: conflict-free LDS.128 (K = 12 fp32 / 24 bf16 timesteps per lane)
+    // odd: conflict-free LDS.128 (K = 12 fp32 / 24 bf16 timesteps per lane; K = 20 with one
+    // chain measured slower: cfg4 0.906 vs 0.818 ms)
+    constexpr int kNv = 3;
     using S = WarpRowTmaSmem<T, kNv * kVec>;
     constexpr int kNu = sizeof(T) == 2 ? 1 : 2;  // K = 24 leaves no registers for a second chain
     auto kern = selective_scan_warp_row_tma_kernel<T, kVec, kNv, kNu>;

@@ -26,7 +26,8 @@ template <typename T, int K>
 struct WarpRowTmaSmem {
     static constexpr int N = 16;
     static constexpr int kTileT = 32 * K;                    // timesteps per warp tile
-    static constexpr int kBoxT = kTileT / 3;                 // TMA box: <= 256 elements per dim
+    static constexpr int kNv = K * static_cast<int>(sizeof(T)) / 16;  // 128-bit vectors per lane
+    static constexpr int kBoxT = kTileT / kNv;               // TMA box: <= 256 elements per dim
     static constexpr int kBoxes = kTileT / kBoxT;            // boxes per tensor per tile
     static constexpr int kBoxBytes = N * kBoxT * static_cast<int>(sizeof(T));
     static constexpr int kStageBytes = 2 * kBoxes * kBoxBytes;  // B boxes then C boxes

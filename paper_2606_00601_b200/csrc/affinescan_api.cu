@@ -57,6 +57,7 @@ struct Buffer {
     size_t bytes = 0;
 };
 std::mutex g_mu;
+std::mutex g_host_mu;  // the _host entry points share the per-device staging buffers
 std::map<std::pair<int, void*>, Buffer> g_scratch;  // (device, stream) -> look-back scratch
 std::map<std::pair<int, int>, Buffer> g_staging;    // (device, slot)   -> host-API staging
 
@@ -555,6 +556,7 @@ int affine_scan_host(const void* a, const void* u, const float* h0, void* h, flo
         return AFFINESCAN_ERR_SHAPE;
     if (total > 0 && (!a || !u || !h)) return AFFINESCAN_ERR_NULL;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    std::lock_guard<std::mutex> host_lock(g_host_mu);
     const size_t eb = static_cast<size_t>(total) * elt_size(io_dtype);
     const size_t sb = static_cast<size_t>(num_seq) * sizeof(float);
     void *da, *du, *dh0, *dh, *dhl;
@@ -606,6 +608,7 @@ int selective_scan_fwd_host(const void* x, const void* delta, const float* A, co
         return AFFINESCAN_ERR_SHAPE;
     if (total > 0 && (!x || !delta || !A || !B || !C || !y)) return AFFINESCAN_ERR_NULL;
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    std::lock_guard<std::mutex> host_lock(g_host_mu);
     const size_t es = elt_size(io_dtype);
     const size_t xb = static_cast<size_t>(total) * es;
     const size_t bb = static_cast<size_t>(bnl) * es;

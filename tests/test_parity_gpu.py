@@ -467,3 +467,30 @@ def test_config5_affine_bandwidth_sweep_sampled_sequences(cuda_device):
             res = (hb - (a[s0:s1].double() * prev + u[s0:s1].double())).abs() / (1 + hb.abs())
             worst = max(worst, res.max().item())
         assert worst <= 1e-5, f"cfg5 L=2^{logL}: recurrence residual {worst:.2e}"
+
+
+# ============================================================ seeded random shapes (fuzz)
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_random_shapes_every_variant_against_the_oracle(cuda_device, seed):
+    """Seeded random small shapes (ragged L, odd row counts, optional D / h0) through every
+    schedule that accepts them; outputs are NaN-prefilled, so an unwritten element fails."""
+    rng = np.random.default_rng(seed)
+    for _ in range(6):
+        dtype = DTYPES[int(rng.integers(2))]
+        vec = 4 if dtype == torch.float32 else 8
+        batch = int(rng.integers(1, 4))
+        L = int(rng.integers(1, 90)) * vec
+        d_inner = int(rng.integers(1, 70))
+        inp = _selective_inputs(batch, d_inner, 16, L, dtype, cuda_device, int(rng.integers(1 << 20)),
+                                with_D=bool(rng.integers(2)), with_h0=bool(rng.integers(2)))
+        for v in (lib.VARIANT_AUTO, lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_WARP_ROW_TMA):
+            check_selective(inp, v, f"fuzz {batch}x{d_inner}x{L} {dtype} v{v}")
+        d32 = 32 * int(rng.integers(1, 4))
+        inp = _selective_inputs(batch, d32, 16, L, dtype, cuda_device, int(rng.integers(1 << 20)),
+                                with_D=bool(rng.integers(2)), with_h0=bool(rng.integers(2)))
+        check_selective(inp, lib.SELECTIVE_LANE_ROW, f"fuzz lane_row {batch}x{d32}x{L} {dtype}")
+        S, La = int(rng.integers(1, 40)), int(rng.integers(1, 9000))
+        ainp = _affine_inputs(S, La, dtype, cuda_device, int(rng.integers(1 << 20)),
+                              with_h0=bool(rng.integers(2)))
+        for v in [lib.VARIANT_AUTO] + AFFINE_VARIANTS:
+            check_affine(ainp, v, f"fuzz affine {S}x{La} {dtype} v{v}")

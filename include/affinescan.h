@@ -156,7 +156,9 @@ AFFINESCAN_API int selective_scan_fwd_ex(const void* x, const void* delta, const
                                          int d_inner, int N, int64_t L, int io_dtype,
                                          int variant, void* cuda_stream);
 
-/* Same computation with HOST buffers (see affine_scan_host). */
+/* Same computation with HOST buffers (see affine_scan_host).  Pipelined over batches: the H2D
+ * copy of batch b+1, the kernel of batch b and the D2H copy of batch b-1 overlap on internal
+ * copy streams (pinned host memory is needed for the overlap; pageable memory still works). */
 AFFINESCAN_API int selective_scan_fwd_host(const void* x, const void* delta, const float* A,
                                            const void* B, const void* C, const float* D,
                                            const float* h0, void* y, float* h_last,

@@ -521,6 +521,29 @@ int stage_in(int slot, const void* host, size_t bytes, cudaStream_t stream, void
     return AFFINESCAN_OK;
 }
 
+// Copy-in / copy-out streams and events of the pipelined _host entry point (per device).
+struct HostPipe {
+    cudaStream_t in = nullptr, out = nullptr;
+    cudaEvent_t start = nullptr;
+    std::vector<cudaEvent_t> in_done, k_done;
+};
+std::map<int, HostPipe> g_pipes;
+
+int get_host_pipe(HostPipe** out)
+{
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_mu);
+    HostPipe& p = g_pipes[dev];
+    if (!p.in) {
+        AS_CUDA(cudaStreamCreateWithFlags(&p.in, cudaStreamNonBlocking));
+        AS_CUDA(cudaStreamCreateWithFlags(&p.out, cudaStreamNonBlocking));
+        AS_CUDA(cudaEventCreateWithFlags(&p.start, cudaEventDisableTiming));
+    }
+    *out = &p;
+    return AFFINESCAN_OK;
+}
+
 int stage_out_alloc(int slot, const void* host, size_t bytes, void** dev)
 {
     *dev = nullptr;
@@ -617,22 +640,73 @@ int selective_scan_fwd_host(const void* x, const void* delta, const float* A, co
     const size_t hb = static_cast<size_t>(rows) * N * sizeof(float);
     void *dx, *dd, *dA, *dB, *dC, *dD, *dh0, *dy, *dhl;
     int st;
-    if ((st = stage_in(10, x, xb, stream, &dx)) != AFFINESCAN_OK) return st;
-    if ((st = stage_in(11, delta, xb, stream, &dd)) != AFFINESCAN_OK) return st;
+    // Device staging (cached, full size), then a three-stage pipeline over batches:
+    // H2D of batch b+1 (copy-in stream) || kernel of batch b (caller's stream) || D2H of batch
+    // b-1 (copy-out stream).  PCIe is full duplex, so the step costs ~max(H2D, D2H), not the sum.
+    if ((st = get_staging(10, xb, &dx)) != AFFINESCAN_OK) return st;
+    if ((st = get_staging(11, xb, &dd)) != AFFINESCAN_OK) return st;
     if ((st = stage_in(12, A, ab, stream, &dA)) != AFFINESCAN_OK) return st;
-    if ((st = stage_in(13, B, bb, stream, &dB)) != AFFINESCAN_OK) return st;
-    if ((st = stage_in(14, C, bb, stream, &dC)) != AFFINESCAN_OK) return st;
+    if ((st = get_staging(13, bb, &dB)) != AFFINESCAN_OK) return st;
+    if ((st = get_staging(14, bb, &dC)) != AFFINESCAN_OK) return st;
     if ((st = stage_in(15, D, db, stream, &dD)) != AFFINESCAN_OK) return st;
     if ((st = stage_in(16, h0, hb, stream, &dh0)) != AFFINESCAN_OK) return st;
     if ((st = stage_out_alloc(17, y, xb, &dy)) != AFFINESCAN_OK) return st;
     if ((st = stage_out_alloc(18, h_last, hb, &dhl)) != AFFINESCAN_OK) return st;
-    st = selective_scan_impl(dx, dd, static_cast<const float*>(dA), dB, dC,
-                             static_cast<const float*>(dD), static_cast<const float*>(dh0), dy,
-                             static_cast<float*>(dhl), batch, d_inner, N, L, io_dtype,
-                             AFFINESCAN_VARIANT_AUTO, cuda_stream);
-    if (st != AFFINESCAN_OK) return st;
-    if (y && xb) AS_CUDA(cudaMemcpyAsync(y, dy, xb, cudaMemcpyDeviceToHost, stream));
-    if (h_last && hb) AS_CUDA(cudaMemcpyAsync(h_last, dhl, hb, cudaMemcpyDeviceToHost, stream));
+    if (total == 0) {
+        AS_CUDA(cudaStreamSynchronize(stream));
+        return AFFINESCAN_OK;
+    }
+    HostPipe* pipe = nullptr;
+    if ((st = get_host_pipe(&pipe)) != AFFINESCAN_OK) return st;
+    // batches per chunk: at least ~16 MB of x per chunk so that copies stay at full PCIe rate
+    const size_t xb1 = xb / batch, bb1 = bb / batch, hb1 = hb / batch;
+    int per = static_cast<int>((16u << 20) / (xb1 ? xb1 : 1)) + 1;
+    if (per > batch) per = batch;
+    const int nchunks = (batch + per - 1) / per;
+    if (static_cast<int>(pipe->in_done.size()) < nchunks) {
+        const size_t old = pipe->in_done.size();
+        pipe->in_done.resize(nchunks);
+        pipe->k_done.resize(nchunks);
+        for (size_t i = old; i < pipe->in_done.size(); ++i) {
+            AS_CUDA(cudaEventCreateWithFlags(&pipe->in_done[i], cudaEventDisableTiming));
+            AS_CUDA(cudaEventCreateWithFlags(&pipe->k_done[i], cudaEventDisableTiming));
+        }
+    }
+    // the small per-call tensors (A, D, h0) went in on the caller's stream: the copy streams must
+    // not overtake an earlier call's use of the staging buffers either
+    AS_CUDA(cudaEventRecord(pipe->start, stream));
+    AS_CUDA(cudaStreamWaitEvent(pipe->in, pipe->start, 0));
+    AS_CUDA(cudaStreamWaitEvent(pipe->out, pipe->start, 0));
+    auto off = [](const void* p, size_t bytes) {
+        return static_cast<const void*>(static_cast<const unsigned char*>(p) + bytes);
+    };
+    auto offm = [](void* p, size_t bytes) {
+        return static_cast<void*>(static_cast<unsigned char*>(p) + bytes);
+    };
+    for (int c = 0; c < nchunks; ++c) {
+        const int b0 = c * per;
+        const int nb = (b0 + per <= batch) ? per : batch - b0;
+        const size_t xo = xb1 * b0, bo = bb1 * b0, ho = hb1 * b0;
+        AS_CUDA(cudaMemcpyAsync(offm(dx, xo), off(x, xo), xb1 * nb, cudaMemcpyHostToDevice, pipe->in));
+        AS_CUDA(cudaMemcpyAsync(offm(dd, xo), off(delta, xo), xb1 * nb, cudaMemcpyHostToDevice, pipe->in));
+        AS_CUDA(cudaMemcpyAsync(offm(dB, bo), off(B, bo), bb1 * nb, cudaMemcpyHostToDevice, pipe->in));
+        AS_CUDA(cudaMemcpyAsync(offm(dC, bo), off(C, bo), bb1 * nb, cudaMemcpyHostToDevice, pipe->in));
+        AS_CUDA(cudaEventRecord(pipe->in_done[c], pipe->in));
+        AS_CUDA(cudaStreamWaitEvent(stream, pipe->in_done[c], 0));
+        st = selective_scan_impl(offm(dx, xo), offm(dd, xo), static_cast<const float*>(dA),
+                                 offm(dB, bo), offm(dC, bo), static_cast<const float*>(dD),
+                                 dh0 ? static_cast<const float*>(offm(dh0, ho)) : nullptr,
+                                 offm(dy, xo), dhl ? static_cast<float*>(offm(dhl, ho)) : nullptr, nb,
+                                 d_inner, N, L, io_dtype, AFFINESCAN_VARIANT_AUTO, cuda_stream);
+        if (st != AFFINESCAN_OK) return st;
+        AS_CUDA(cudaEventRecord(pipe->k_done[c], stream));
+        AS_CUDA(cudaStreamWaitEvent(pipe->out, pipe->k_done[c], 0));
+        AS_CUDA(cudaMemcpyAsync(offm(y, xo), off(dy, xo), xb1 * nb, cudaMemcpyDeviceToHost, pipe->out));
+        if (h_last)
+            AS_CUDA(cudaMemcpyAsync(offm(h_last, ho), off(dhl, ho), hb1 * nb, cudaMemcpyDeviceToHost,
+                                    pipe->out));
+    }
+    AS_CUDA(cudaStreamSynchronize(pipe->out));
     AS_CUDA(cudaStreamSynchronize(stream));
     return AFFINESCAN_OK;
 }

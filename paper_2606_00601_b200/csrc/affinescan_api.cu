@@ -584,16 +584,67 @@ int affine_scan_host(const void* a, const void* u, const float* h0, void* h, flo
     const size_t sb = static_cast<size_t>(num_seq) * sizeof(float);
     void *da, *du, *dh0, *dh, *dhl;
     int st;
-    if ((st = stage_in(0, a, eb, stream, &da)) != AFFINESCAN_OK) return st;
-    if ((st = stage_in(1, u, eb, stream, &du)) != AFFINESCAN_OK) return st;
+    // same three-stage pipeline as selective_scan_fwd_host, over chunks of whole sequences
+    if ((st = get_staging(0, eb, &da)) != AFFINESCAN_OK) return st;
+    if ((st = get_staging(1, eb, &du)) != AFFINESCAN_OK) return st;
     if ((st = stage_in(2, h0, sb, stream, &dh0)) != AFFINESCAN_OK) return st;
     if ((st = stage_out_alloc(3, h, eb, &dh)) != AFFINESCAN_OK) return st;
     if ((st = stage_out_alloc(4, h_last, sb, &dhl)) != AFFINESCAN_OK) return st;
-    st = affine_scan_impl(da, du, static_cast<const float*>(dh0), dh, static_cast<float*>(dhl),
-                          num_seq, L, io_dtype, AFFINESCAN_VARIANT_AUTO, cuda_stream);
-    if (st != AFFINESCAN_OK) return st;
-    if (h && eb) AS_CUDA(cudaMemcpyAsync(h, dh, eb, cudaMemcpyDeviceToHost, stream));
-    if (h_last && sb) AS_CUDA(cudaMemcpyAsync(h_last, dhl, sb, cudaMemcpyDeviceToHost, stream));
+    if (total == 0) {  // nothing to scan: h_last <- h0 (or 0)
+        st = affine_scan_impl(da, du, static_cast<const float*>(dh0), dh, static_cast<float*>(dhl),
+                              num_seq, L, io_dtype, AFFINESCAN_VARIANT_AUTO, cuda_stream);
+        if (st != AFFINESCAN_OK) return st;
+        if (h_last && sb) AS_CUDA(cudaMemcpyAsync(h_last, dhl, sb, cudaMemcpyDeviceToHost, stream));
+        AS_CUDA(cudaStreamSynchronize(stream));
+        return AFFINESCAN_OK;
+    }
+    HostPipe* pipe = nullptr;
+    if ((st = get_host_pipe(&pipe)) != AFFINESCAN_OK) return st;
+    const size_t seq_bytes = static_cast<size_t>(L) * elt_size(io_dtype);
+    int64_t per = static_cast<int64_t>((16u << 20) / seq_bytes) + 1;  // sequences per chunk
+    if (per > num_seq) per = num_seq;
+    int64_t nchunks = (num_seq + per - 1) / per;
+    if (nchunks > 64) {  // bound the number of events
+        nchunks = 64;
+        per = (num_seq + nchunks - 1) / nchunks;
+        nchunks = (num_seq + per - 1) / per;
+    }
+    if (static_cast<int64_t>(pipe->in_done.size()) < nchunks) {
+        const size_t old = pipe->in_done.size();
+        pipe->in_done.resize(nchunks);
+        pipe->k_done.resize(nchunks);
+        for (size_t i = old; i < pipe->in_done.size(); ++i) {
+            AS_CUDA(cudaEventCreateWithFlags(&pipe->in_done[i], cudaEventDisableTiming));
+            AS_CUDA(cudaEventCreateWithFlags(&pipe->k_done[i], cudaEventDisableTiming));
+        }
+    }
+    AS_CUDA(cudaEventRecord(pipe->start, stream));
+    AS_CUDA(cudaStreamWaitEvent(pipe->in, pipe->start, 0));
+    AS_CUDA(cudaStreamWaitEvent(pipe->out, pipe->start, 0));
+    auto at = [](const void* p, size_t bytes) {
+        return const_cast<void*>(static_cast<const void*>(static_cast<const unsigned char*>(p) + bytes));
+    };
+    for (int64_t c = 0; c < nchunks; ++c) {
+        const int64_t s0 = c * per;
+        const int64_t ns = (s0 + per <= num_seq) ? per : num_seq - s0;
+        const size_t eo = seq_bytes * s0, so = sizeof(float) * s0;
+        AS_CUDA(cudaMemcpyAsync(at(da, eo), at(a, eo), seq_bytes * ns, cudaMemcpyHostToDevice, pipe->in));
+        AS_CUDA(cudaMemcpyAsync(at(du, eo), at(u, eo), seq_bytes * ns, cudaMemcpyHostToDevice, pipe->in));
+        AS_CUDA(cudaEventRecord(pipe->in_done[c], pipe->in));
+        AS_CUDA(cudaStreamWaitEvent(stream, pipe->in_done[c], 0));
+        st = affine_scan_impl(at(da, eo), at(du, eo),
+                              dh0 ? static_cast<const float*>(at(dh0, so)) : nullptr, at(dh, eo),
+                              dhl ? static_cast<float*>(at(dhl, so)) : nullptr, ns, L, io_dtype,
+                              AFFINESCAN_VARIANT_AUTO, cuda_stream);
+        if (st != AFFINESCAN_OK) return st;
+        AS_CUDA(cudaEventRecord(pipe->k_done[c], stream));
+        AS_CUDA(cudaStreamWaitEvent(pipe->out, pipe->k_done[c], 0));
+        AS_CUDA(cudaMemcpyAsync(at(h, eo), at(dh, eo), seq_bytes * ns, cudaMemcpyDeviceToHost, pipe->out));
+        if (h_last)
+            AS_CUDA(cudaMemcpyAsync(at(h_last, so), at(dhl, so), sizeof(float) * ns,
+                                    cudaMemcpyDeviceToHost, pipe->out));
+    }
+    AS_CUDA(cudaStreamSynchronize(pipe->out));
     AS_CUDA(cudaStreamSynchronize(stream));
     return AFFINESCAN_OK;
 }

@@ -184,6 +184,24 @@ def test_affine_host_api_matches_device_api(cuda_device):
     assert torch.equal(hh, h.cpu()) and torch.equal(hhl, hl.cpu())
 
 
+def test_affine_host_api_pipelines_over_several_chunks(cuda_device):
+    """> 16 MB per tensor: the host call splits the sequences into chunks that overlap H2D,
+    kernel and D2H; with and without h0 / h_last; a repeated call reuses the staging buffers."""
+    inp = _affine_inputs(45, 200000, torch.float32, cuda_device, 14, a_lo=0.9, a_hi=0.9999)
+    h, hl = gpu_affine(inp)
+    a, u, h0 = inp["a"].cpu().pin_memory(), inp["u"].cpu().pin_memory(), inp["h0"].cpu()
+    for use_h0, want_hl in ((True, True), (False, False), (True, True)):
+        hh = torch.full_like(a, float("nan")).pin_memory()
+        hhl = torch.full((45,), float("nan")) if want_hl else None
+        lib.affine_scan_host(a, u, h0 if use_h0 else None, hh, hhl)
+        if use_h0:
+            assert rel_err(hh, to_f64_numpy(h)) <= 1e-5
+            assert rel_err(hhl, to_f64_numpy(hl)) <= 1e-5
+        else:
+            href, _ = oracle.affine_scan(to_f64_numpy(a[:3]), to_f64_numpy(u[:3]), None)
+            assert_close(hh[:3], href, torch.float32, "host affine without h0")
+
+
 # ================================================================ selective: T1 shapes
 @pytest.mark.parametrize("dtype", DTYPES)
 def test_selective_warp_row_small_and_ragged_shapes(cuda_device, dtype):
@@ -354,6 +372,27 @@ def test_selective_host_api_matches_device_api(cuda_device):
     lib.selective_scan_fwd_host(host["x"].pin_memory(), host["delta"].pin_memory(), host["A"],
                                 host["B"], host["C"], host["D"], None, yh, hlh)
     assert torch.equal(yh, y.cpu()) and torch.equal(hlh, hl.cpu())
+
+
+def test_selective_host_api_pipelines_over_several_chunks(cuda_device):
+    """x > 16 MB per chunk boundary: batches go through the H2D || kernel || D2H pipeline in
+    several chunks (the chunks may take another schedule than the whole problem would)."""
+    inp = _selective_inputs(5, 64, 16, 20000, torch.float32, cuda_device, 18, with_h0=True)
+    y, hl = gpu_selective(inp)
+    host = {k: (None if v is None else v.cpu().pin_memory()) for k, v in inp.items()}
+    yh = torch.full_like(host["x"], float("nan")).pin_memory()
+    hlh = torch.full((5, 64, 16), float("nan"))
+    lib.selective_scan_fwd_host(host["x"], host["delta"], host["A"], host["B"], host["C"],
+                                host["D"], host["h0"], yh, hlh)
+    assert rel_err(yh, to_f64_numpy(y)) <= 1e-5 and rel_err(hlh, to_f64_numpy(hl)) <= 1e-5
+    yh.fill_(float("nan"))
+    lib.selective_scan_fwd_host(host["x"], host["delta"], host["A"], host["B"], host["C"],
+                                None, None, yh, None)
+    sub = {k: (None if k in ("D", "h0") else v) for k, v in inp.items()}
+    rows = [(0, 0), (2, 63), (4, 17)]
+    yref, _ = oracle_selective_rows(sub, rows)
+    for i, (b, d) in enumerate(rows):
+        assert_close(yh[b, d], yref[i], torch.float32, "host selective without D/h0/h_last")
 
 
 def test_runs_on_a_non_default_stream_and_counts_launches(cuda_device):

@@ -250,6 +250,8 @@ int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, flo
 
 // ============================================================== selective_scan dispatch
 constexpr int kSmCount = 148;
+constexpr int kWarpRowTmaRowsPerWarpF32 = 1;
+constexpr int kWarpRowTmaMaxWarps2 = 7;    // two rows per warp: (7+1) warps x 32 x <= 255 registers
 constexpr int kWarpRowTmaMaxWarps = 11;   // warp_row_tma: rows per CTA (+1 producer warp = 384 threads)
 constexpr int64_t kWarpRowTmaMinL = 1024; // below two warp tiles the plain warp_row is as good
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
@@ -405,8 +407,12 @@ int launch_warp_row_tma(const T* x, const T* delta, const float* A, const T* B, 
     // chain measured slower: cfg4 0.906 vs 0.818 ms)
     constexpr int kNv = 3;
     using S = WarpRowTmaSmem<T, kNv * kVec>;
-    constexpr int kNu = sizeof(T) == 2 ? 1 : 2;  // K = 24 leaves no registers for a second chain
-    auto kern = selective_scan_warp_row_tma_kernel<T, kVec, kNv, kNu>;
+    // chains per warp = NU states x RW rows.  fp32 io: two states of one row (two rows per warp
+    // sharing every LDS.128 of B_t/C_t halve the shared-memory traffic but leave 6 warps per SM:
+    // cfg4 1.14 vs 0.82 ms); bf16 io: K = 24 leaves registers for one chain only.
+    constexpr int kRw = sizeof(T) == 2 ? 1 : kWarpRowTmaRowsPerWarpF32;
+    constexpr int kNu = (sizeof(T) == 2 || kRw == 2) ? 1 : 2;
+    auto kern = selective_scan_warp_row_tma_kernel<T, kVec, kNv, kNu, kRw>;
     static std::atomic<unsigned> configured{0};  // bit per device
     int dev = 0;
     AS_CUDA(cudaGetDevice(&dev));
@@ -422,9 +428,10 @@ int launch_warp_row_tma(const T* x, const T* delta, const float* A, const T* B, 
     // R rows (warps) of one batch per CTA, sized so that one wave of CTAs covers all rows when
     // they fit (cfg2/cfg4: 1536 rows -> 140 CTAs of 11 warps on 148 SMs)
     const int slots = kSmCount / batch > 0 ? kSmCount / batch : 1;
-    int R = (d_inner + slots - 1) / slots;
-    R = R < 1 ? 1 : (R > kWarpRowTmaMaxWarps ? kWarpRowTmaMaxWarps : R);
-    const int ctas_per_batch = (d_inner + R - 1) / R;
+    const int max_warps = kRw == 1 ? kWarpRowTmaMaxWarps : kWarpRowTmaMaxWarps2;
+    int R = ((d_inner + slots - 1) / slots + kRw - 1) / kRw;  // consumer warps per CTA
+    R = R < 1 ? 1 : (R > max_warps ? max_warps : R);
+    const int ctas_per_batch = (d_inner + R * kRw - 1) / (R * kRw);
     const int64_t blocks = static_cast<int64_t>(batch) * ctas_per_batch;
     if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
     kern<<<static_cast<unsigned>(blocks), (R + 1) * 32, S::kBytes, stream>>>(

@@ -60,9 +60,11 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
-// NU = states processed together per n-iteration (independent chains for ILP).
-template <typename T, int VEC, int NV, int NU>
-__global__ void __launch_bounds__(384, 1)
+// NU = states processed together per n-iteration, RW = rows per warp: NU*RW independent chains
+// per warp; the RW rows of a warp share every LDS of B_t/C_t (half the shared-memory traffic
+// per state-step at RW = 2).
+template <typename T, int VEC, int NV, int NU, int RW>
+__global__ void __launch_bounds__(RW == 1 ? 384 : 256, 1)
 selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                    const float* __restrict__ A,
                                    const __grid_constant__ CUtensorMap mapB,
@@ -82,13 +84,19 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
-    const int R = (blockDim.x >> 5) - 1;  // rows (consumer warps) per CTA; warp R is the producer
+    const int R = (blockDim.x >> 5) - 1;  // consumer warps per CTA; warp R is the producer
     const int b = blockIdx.x / ctas_per_batch;
-    const int d0 = (blockIdx.x - b * ctas_per_batch) * R;
-    const int d = d0 + warp;
-    const bool active = d < d_inner;  // inactive warps still take part in the stage ring
-    const int dd = active ? d : d_inner - 1;
-    const long long row = static_cast<long long>(b) * d_inner + dd;
+    const int d0 = (blockIdx.x - b * ctas_per_batch) * R * RW;
+    bool active[RW];   // inactive rows are computed (on a valid row) but never stored: their
+    int dd[RW];        // warps still take part in the stage ring
+    long long row[RW];
+#pragma unroll
+    for (int r = 0; r < RW; ++r) {
+        const int d = d0 + warp * RW + r;
+        active[r] = d < d_inner;
+        dd[r] = active[r] ? d : d_inner - 1;
+        row[r] = static_cast<long long>(b) * d_inner + dd[r];
+    }
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -130,14 +138,14 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
         return;
     }
 
-    const T* xr = x + row * L;
-    const T* dr = delta + row * L;
-    T* yr = y + row * L;
-
-    // Lane n keeps A2[n] = A[d,n]*log2(e) and the carry h_in[n]; broadcast by shuffle.
-    float A2r = lane < N ? __ldg(A + static_cast<long long>(dd) * N + lane) * kLog2e : 0.0f;
-    float hcr = (lane < N && h0) ? __ldg(h0 + row * N + lane) : 0.0f;
-    const float Dd = D ? __ldg(D + dd) : 0.0f;
+    // Lane n keeps A2[n] = A[d,n]*log2(e) and the carry h_in[n] of each row; broadcast by shuffle.
+    float A2r[RW], hcr[RW], Dd[RW];
+#pragma unroll
+    for (int r = 0; r < RW; ++r) {
+        A2r[r] = lane < N ? __ldg(A + static_cast<long long>(dd[r]) * N + lane) * kLog2e : 0.0f;
+        hcr[r] = (lane < N && h0) ? __ldg(h0 + row[r] * N + lane) : 0.0f;
+        Dd[r] = D ? __ldg(D + dd[r]) : 0.0f;
+    }
 
     // byte offset (inside a tensor's stage, state n = 0) of this lane's v-th 128-bit vector
     int voff[NV];
@@ -148,16 +156,20 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
     }
 
     // A1: raw 128-bit prefetch of the lane's K timesteps of x and delta, one tile ahead
-    uint4 xq[NV], dq[NV];
+    uint4 xq[RW][NV], dq[RW][NV];
     auto prefetch = [&](long long tile) {
         const long long tl = tile * S::kTileT + lane * K;
 #pragma unroll
-        for (int v = 0; v < NV; ++v) {
-            xq[v] = make_uint4(0, 0, 0, 0);  // identity padding: delta = 0 => a = 1, u = 0 (Q12)
-            dq[v] = make_uint4(0, 0, 0, 0);
-            if (tl + v * VEC < L) {
-                xq[v] = __ldcs(reinterpret_cast<const uint4*>(xr + tl + v * VEC));
-                dq[v] = __ldcs(reinterpret_cast<const uint4*>(dr + tl + v * VEC));
+        for (int r = 0; r < RW; ++r) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                xq[r][v] = make_uint4(0, 0, 0, 0);  // identity padding: delta = 0 => a = 1, u = 0
+                dq[r][v] = make_uint4(0, 0, 0, 0);  // (Q12)
+                if (tl + v * VEC < L) {
+                    xq[r][v] = __ldcs(reinterpret_cast<const uint4*>(x + row[r] * L + tl + v * VEC));
+                    dq[r][v] =
+                        __ldcs(reinterpret_cast<const uint4*>(delta + row[r] * L + tl + v * VEC));
+                }
             }
         }
     };
@@ -167,23 +179,26 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
         const int st = static_cast<int>(tile % S::kStages);
         const unsigned parity = static_cast<unsigned>((tile / S::kStages) & 1);
         const long long tl = tile * S::kTileT + lane * K;  // first timestep of this lane
-        float dl[K], dx[K], yv[K];
+        float dl[RW][K], dx[RW][K], yv[RW][K], dsum[RW];
 #pragma unroll
-        for (int v = 0; v < NV; ++v) {
-            float xv[VEC], dv[VEC];
-            unpack128<T>(xq[v], xv);
-            unpack128<T>(dq[v], dv);
+        for (int r = 0; r < RW; ++r) {
 #pragma unroll
-            for (int k = 0; k < VEC; ++k) {
-                dl[v * VEC + k] = dv[k];
-                dx[v * VEC + k] = dv[k] * xv[k];
-                yv[v * VEC + k] = Dd * xv[k];
+            for (int v = 0; v < NV; ++v) {
+                float xv[VEC], dv[VEC];
+                unpack128<T>(xq[r][v], xv);
+                unpack128<T>(dq[r][v], dv);
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    dl[r][v * VEC + k] = dv[k];
+                    dx[r][v * VEC + k] = dv[k] * xv[k];
+                    yv[r][v * VEC + k] = Dd[r] * xv[k];
+                }
             }
+            dsum[r] = 0.0f;
+#pragma unroll
+            for (int k = 0; k < K; ++k) dsum[r] += dl[r][k];
         }
         if (tile + 1 < ntiles) prefetch(tile + 1);
-        float dsum = 0.0f;
-#pragma unroll
-        for (int k = 0; k < K; ++k) dsum += dl[k];
 
         mbar_wait(&full[st], parity);
         const unsigned char* sB = smem_raw + st * S::kStageBytes;
@@ -191,88 +206,117 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
 
 #pragma unroll 1
         for (int n0 = 0; n0 < N; n0 += NU) {
-            float a[NU][K], u[NU][K];
-            Pair loc[NU];
-            float hin[NU];
-            // ---- A3 + A4 for NU states: independent work, issued back to back
+            float a[NU][RW][K], u[NU][RW][K];
+            Pair inc[NU][RW];
+            float hin[NU][RW];
+            // ---- A3 + A4 for NU states x RW rows: independent work, issued back to back
 #pragma unroll
             for (int j = 0; j < NU; ++j) {
                 const int n = n0 + j;
-                const float A2n = __shfl_sync(kFullMask, A2r, n);
-                hin[j] = __shfl_sync(kFullMask, hcr, n);
+                float A2n[RW];
+#pragma unroll
+                for (int r = 0; r < RW; ++r) {
+                    A2n[r] = __shfl_sync(kFullMask, A2r[r], n);
+                    hin[j][r] = __shfl_sync(kFullMask, hcr[r], n);
+                }
                 const unsigned char* bn = sB + n * S::kBoxT * static_cast<int>(sizeof(T));
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
-                    float bv[VEC];
+                    float bv[VEC];  // one LDS.128 of B serves all RW rows
                     unpack128<T>(*reinterpret_cast<const uint4*>(bn + voff[v]), bv);
 #pragma unroll
-                    for (int k = 0; k < VEC; ++k) {
-                        a[j][v * VEC + k] = ex2_approx(dl[v * VEC + k] * A2n);
-                        u[j][v * VEC + k] = dx[v * VEC + k] * bv[k];
+                    for (int r = 0; r < RW; ++r) {
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            a[j][r][v * VEC + k] = ex2_approx(dl[r][v * VEC + k] * A2n[r]);
+                            u[j][r][v * VEC + k] = dx[r][v * VEC + k] * bv[k];
+                        }
                     }
                 }
-                loc[j] = Pair{ex2_approx(dsum * A2n), u[j][0]};
+#pragma unroll
+                for (int r = 0; r < RW; ++r)
+                    inc[j][r] = Pair{ex2_approx(dsum[r] * A2n[r]), u[j][r][0]};
             }
 #pragma unroll
             for (int k = 1; k < K; ++k) {
 #pragma unroll
-                for (int j = 0; j < NU; ++j) loc[j].U = fmaf(a[j][k], loc[j].U, u[j][k]);
-            }
-            // ---- A5: warp combine (NU interleaved Kogge–Stone scans)
-            Pair inc[NU];
+                for (int j = 0; j < NU; ++j) {
 #pragma unroll
-            for (int j = 0; j < NU; ++j) inc[j] = loc[j];
+                    for (int r = 0; r < RW; ++r)
+                        inc[j][r].U = fmaf(a[j][r][k], inc[j][r].U, u[j][r][k]);
+                }
+            }
+            // ---- A5: warp combine (NU*RW interleaved Kogge–Stone scans)
 #pragma unroll
             for (int dlt = 1; dlt < 32; dlt <<= 1) {
-                Pair pv[NU];
+                Pair pv[NU][RW];
 #pragma unroll
-                for (int j = 0; j < NU; ++j) pv[j] = shfl_up_pair(inc[j], dlt);
+                for (int j = 0; j < NU; ++j) {
+#pragma unroll
+                    for (int r = 0; r < RW; ++r) pv[j][r] = shfl_up_pair(inc[j][r], dlt);
+                }
                 if (lane >= dlt) {
 #pragma unroll
-                    for (int j = 0; j < NU; ++j) inc[j] = compose(inc[j], pv[j]);
+                    for (int j = 0; j < NU; ++j) {
+#pragma unroll
+                        for (int r = 0; r < RW; ++r) inc[j][r] = compose(inc[j][r], pv[j][r]);
+                    }
                 }
             }
             // ---- A7/A8: carry-in, rescan; A9: y accumulation
 #pragma unroll
             for (int j = 0; j < NU; ++j) {
                 const int n = n0 + j;
-                Pair ex = shfl_up_pair(inc[j], 1);
-                if (lane == 0) ex = identity_pair();
-                const Pair tot = shfl_pair(inc[j], 31);
-                float hv = apply(ex, hin[j]);
+                float hv[RW];
+#pragma unroll
+                for (int r = 0; r < RW; ++r) {
+                    Pair ex = shfl_up_pair(inc[j][r], 1);
+                    if (lane == 0) ex = identity_pair();
+                    const Pair tot = shfl_pair(inc[j][r], 31);
+                    hv[r] = apply(ex, hin[j][r]);
+                    const float hout = apply(tot, hin[j][r]);  // state after the tile (uniform)
+                    if (lane == n) hcr[r] = hout;
+                }
                 const unsigned char* cn = sC + n * S::kBoxT * static_cast<int>(sizeof(T));
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
-                    float cc[VEC];
+                    float cc[VEC];  // one LDS.128 of C serves all RW rows
                     unpack128<T>(*reinterpret_cast<const uint4*>(cn + voff[v]), cc);
 #pragma unroll
-                    for (int k = 0; k < VEC; ++k) {
-                        hv = fmaf(a[j][v * VEC + k], hv, u[j][v * VEC + k]);
-                        yv[v * VEC + k] = fmaf(cc[k], hv, yv[v * VEC + k]);
+                    for (int r = 0; r < RW; ++r) {
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            hv[r] = fmaf(a[j][r][v * VEC + k], hv[r], u[j][r][v * VEC + k]);
+                            yv[r][v * VEC + k] = fmaf(cc[k], hv[r], yv[r][v * VEC + k]);
+                        }
                     }
                 }
-                const float hout = apply(tot, hin[j]);  // state after the tile (uniform)
-                if (lane == n) hcr = hout;
             }
         }
         // release the stage; the producer warp refills it with tile + 2 once every warp has
         __syncwarp();
         if (lane == 0) mbar_arrive(&empty[st]);
         // ---- A9: store y
-        if (active) {
 #pragma unroll
-            for (int v = 0; v < NV; ++v) {
-                if (tl + v * VEC < L) {
-                    float out[VEC];
+        for (int r = 0; r < RW; ++r) {
+            if (active[r]) {
 #pragma unroll
-                    for (int k = 0; k < VEC; ++k) out[k] = yv[v * VEC + k];
-                    AccS::store(yr + tl + v * VEC, out);
+                for (int v = 0; v < NV; ++v) {
+                    if (tl + v * VEC < L) {
+                        float out[VEC];
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) out[k] = yv[r][v * VEC + k];
+                        AccS::store(y + row[r] * L + tl + v * VEC, out);
+                    }
                 }
             }
         }
     }
     // ---- A10: final state
-    if (h_last && active && lane < N) h_last[row * N + lane] = hcr;
+#pragma unroll
+    for (int r = 0; r < RW; ++r) {
+        if (h_last && active[r] && lane < N) h_last[row[r] * N + lane] = hcr[r];
+    }
 }
 
 }  // namespace affinescan

@@ -341,6 +341,9 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=device)
     from paper_2606_00601_b200.sharding import max_over_ranks
 
+    from paper_2606_00601_b200 import build as libbuild
+    if not os.path.exists(libbuild.LIB_PATH):
+        libbuild.build()             # fresh checkout: the built library is git-ignored
     import paper_2606_00601_b200 as lib
     lib.set_option(lib.OPT_LANE_ROW_G, args.lane_row_g)
     lib.set_option(lib.OPT_LANE_ROW_POLY16, args.lane_row_poly16)

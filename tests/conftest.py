@@ -10,6 +10,10 @@ if ROOT not in sys.path:
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    # The built library is git-ignored: compile it (nvcc, ~40 s) when a fresh checkout lacks it.
+    from paper_2606_00601_b200 import build as libbuild
+    if not os.path.exists(libbuild.LIB_PATH):
+        libbuild.build()
 
 
 @pytest.fixture(scope="session")

@@ -191,7 +191,11 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
                 unsigned st = kDescInclusive;  // before the stream: state 0
                 if (idx >= 0) {
                     const unsigned long long* d = desc + 2ull * idx;
-                    do { st = desc_load(d, e); } while (st == kDescEmpty);
+                    st = desc_load(d, e);
+                    while (st == kDescEmpty) {  // back off: the poll competes with the data stream
+                        __nanosleep(64);
+                        st = desc_load(d, e);
+                    }
                 }
                 __syncwarp();
                 const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);

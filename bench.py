@@ -36,7 +36,8 @@ FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback ("of fallback")
 NOMINAL_HBM_GBS = 8000.0       # BASELINE.json north_star "~8 TB/s"
 SM_COUNT = 148
 MUFU_PER_CLK_PER_SM = 16       # ex2 results / clk / SM (4 per sub-partition), DESIGN.md §6
-FP32_PER_CLK_PER_SM = 128      # FP32 lane-ops / clk / SM
+FP32_PER_CLK_PER_SM = 128      # FP32 lane-ops / clk / SM (nominal)
+FMA_LANEOPS_PER_CLK_PER_SM = 124   # measured with FFMA2 (profiles/r01a_pipe_probes.md)
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -427,20 +428,42 @@ def run_ours(args):
         "hbm_gbs_achieved": round(achieved, 1),
     }
     if c.kind == "selective":
-        # the binding roofline of this path: exp on the SFU and FP32 lane-ops
+        # The binding roofline of this path is arithmetic, not HBM: one 2^x
+        # and 4 FP32 lane-ops per state-step.  Ceiling with BOTH pipes in use: a share f of the
+        # 2^x goes to the fma pipe as a degree-DEG polynomial (3 + DEG lane-ops instead of the one
+        # argument multiply: 2 + DEG extra), the rest
+        # to the MUFU; the two pipes balance at (1 - f) / 16 = (4 + (2 + DEG) f) / 124 cycles per
+        # state-step per SM (16 MUFU and 124 packed-FP32 lane-ops per clock per SM, measured:
+        # profiles/r01a_pipe_probes.md).
         mhz = clk.get("sm_mhz") or clk.get("sm_max_mhz") or 1965.0
+        deg = 3 if c.dtype == torch.bfloat16 else 5
+        f = (FMA_LANEOPS_PER_CLK_PER_SM - 4 * MUFU_PER_CLK_PER_SM) / (
+            FMA_LANEOPS_PER_CLK_PER_SM + (2 + deg) * MUFU_PER_CLK_PER_SM)
+        per_clk_sm = MUFU_PER_CLK_PER_SM / (1.0 - f)          # state-steps / clk / SM
         steps_state = c.elements * c.N
+        alu_peak = per_clk_sm * SM_COUNT * mhz * 1e6          # state-steps / s
         mufu_ms = steps_state / (MUFU_PER_CLK_PER_SM * SM_COUNT * mhz * 1e6) * 1e3
-        fp32_ms = 4 * steps_state / (FP32_PER_CLK_PER_SM * SM_COUNT * mhz * 1e6) * 1e3
-        line["roofline_alu"] = {
-            "bound": "alu", "unit": "state-steps/s",
-            "achieved": steps_state / (kernel_ms * 1e-3),
-            "peak": steps_state / (mufu_ms * 1e-3),
-            "frac": round(mufu_ms / kernel_ms, 4),
-            "note": "peak = 16 MUFU.EX2/clk/SM x 148 SMs x sampled SM clock, 1 exp per "
-                    "state-step; fp32_wall_ms is 4 FP32 lane-ops per state-step at 128/clk/SM",
-            "mufu_wall_ms": round(mufu_ms, 4), "fp32_wall_ms": round(fp32_ms, 4),
-            "sm_mhz_used": mhz}
+        alu_achieved = steps_state / (kernel_ms * 1e-3)
+        hbm = dict(roofline)
+        line["roofline_hbm"] = hbm                             # the metric's own denominator
+        line["roofline"] = {
+            "bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "state-steps/s",
+            "frac": round(alu_achieved / alu_peak, 4), "traffic": traffic,
+            "peak_kind": "derived: MUFU 16/clk/SM + fma pipe 124 lane-ops/clk/SM (measured "
+                         "probes) x 148 SMs x sampled SM clock, balanced polynomial offload",
+            "poly_share_at_balance": round(f, 4), "state_steps_per_clk_per_sm": round(per_clk_sm, 2),
+            "kernel_ms": hbm["kernel_ms"], "kernel_ms_min": hbm["kernel_ms_min"],
+            "kernel_ms_median": hbm["kernel_ms_median"], "kernel": hbm["kernel"],
+            "algorithmic_bytes": w.bytes,
+            "hbm_frac": hbm["frac"], "hbm_gbs": hbm["achieved"],
+            "mufu_only_wall_ms": round(mufu_ms, 4),
+            "frac_of_mufu_only_wall": round(mufu_ms / kernel_ms, 4),
+            "alu_wall_ms": round(steps_state / alu_peak * 1e3, 4), "sm_mhz_used": mhz}
+        if "ablation" in hbm:
+            line["roofline"]["ablation"] = hbm["ablation"]
+        line["roofline_alu"] = {"frac": line["roofline"]["frac_of_mufu_only_wall"],
+                                "note": "fraction of the all-MUFU wall (1 exp per state-step at "
+                                        "16/clk/SM); see roofline for the two-pipe ceiling"}
 
     # ---- end to end through the C-ABI with host buffers
     if not args.no_e2e:

@@ -820,6 +820,16 @@ int affinescan_release_cache(void)
             it = g_staging.erase(it);
         } else ++it;
     }
+    auto pit = g_pipes.find(dev);  // copy streams / events of the pipelined _host entry points
+    if (pit != g_pipes.end()) {
+        HostPipe& p = pit->second;
+        for (cudaEvent_t e : p.in_done) cudaEventDestroy(e);
+        for (cudaEvent_t e : p.k_done) cudaEventDestroy(e);
+        if (p.start) cudaEventDestroy(p.start);
+        if (p.in) cudaStreamDestroy(p.in);
+        if (p.out) cudaStreamDestroy(p.out);
+        g_pipes.erase(pit);
+    }
     return AFFINESCAN_OK;
 }
 

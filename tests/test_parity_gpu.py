@@ -533,3 +533,18 @@ def test_random_shapes_every_variant_against_the_oracle(cuda_device, seed):
                               with_h0=bool(rng.integers(2)))
         for v in [lib.VARIANT_AUTO] + AFFINE_VARIANTS:
             check_affine(ainp, v, f"fuzz affine {S}x{La} {dtype} v{v}")
+
+
+def test_release_cache_then_calls_still_work(cuda_device):
+    """affinescan_release_cache frees scratch, staging buffers and the host-pipeline streams;
+    the next calls re-create what they need."""
+    inp = _affine_inputs(3, 20000, torch.float32, cuda_device, 41)
+    h, hl = gpu_affine(inp, lib.AFFINE_LOOKBACK)
+    a, u = inp["a"].cpu().pin_memory(), inp["u"].cpu().pin_memory()
+    hh = torch.empty_like(a).pin_memory()
+    lib.affine_scan_host(a, u, inp["h0"].cpu(), hh, None)
+    lib.release_cache()
+    h2, hl2 = gpu_affine(inp, lib.AFFINE_LOOKBACK)
+    hh2 = torch.empty_like(a).pin_memory()
+    lib.affine_scan_host(a, u, inp["h0"].cpu(), hh2, None)
+    assert torch.equal(h, h2) and torch.equal(hl, hl2) and torch.equal(hh, hh2)

@@ -401,8 +401,11 @@ def run_ours(args):
     achieved = w.bytes / (kernel_ms * 1e-3) / 1e9
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as f:
-            traffic = json.load(f).get(c.name)
+        with open(os.path.join(ROOT, "profiles", "traffic.txt")) as f:
+            for ln in f:
+                parts = ln.split()
+                if len(parts) >= 2 and parts[0] == c.name:
+                    traffic = int(parts[1])
     except Exception:
         pass
     clk = clocks.summary()

@@ -13,14 +13,17 @@ import paper_2606_00601_b200 as lib
 from workloads import (config, make_affine_inputs, make_selective_inputs, normal, to_f64_numpy,
                        uniform)
 
-from util import (TOL, assert_close, check_affine, check_selective, gpu_affine, gpu_selective,
-                  lane_row_ok, oracle_affine, oracle_selective, oracle_selective_rows, rel_err)
+from util import (TOL, assert_close, assert_close_all, check_affine, check_selective, gpu_affine,
+                  gpu_selective, host_threads, lane_row_ok, oracle_affine, oracle_selective,
+                  oracle_selective_all_rows, oracle_selective_rows, rel_err, rel_err_device)
 
 pytestmark = pytest.mark.gpu
 
 AFFINE_VARIANTS = [lib.AFFINE_LOOKBACK, lib.AFFINE_CTA_LOOP, lib.AFFINE_BLELLOCH,
                    lib.AFFINE_WARP_SEQ]
 DTYPES = [torch.float32, torch.bfloat16]
+SELECTIVE_VARIANTS = [lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_LANE_ROW, lib.SELECTIVE_WARP_ROW_TMA]
+FEW_ROWS_VARIANTS = [lib.SELECTIVE_WARP_ROW_TMA]      # what AUTO may pick for few rows x long L
 
 
 def _affine_inputs(S, L, dtype, dev, seed, with_h0=True, a_lo=0.5, a_hi=0.99):
@@ -425,87 +428,93 @@ def test_config2_selective_fp32_full(cuda_device):
         assert_close(hl, hlref, torch.float32, f"cfg2 h_last v={v}")
 
 
-def _sample_rows(batch, d_inner, k, seed):
-    rng = np.random.default_rng(seed)
-    rows = {(0, 0), (batch - 1, d_inner - 1), (0, d_inner - 1), (batch - 1, 0)}
-    while len(rows) < k:
-        rows.add((int(rng.integers(batch)), int(rng.integers(d_inner))))
-    return sorted(rows)
-
-
-def _check_selective_sampled(inp, variant, rows, dtype, what):
+def _check_selective_every_element(inp, ref, variant, dtype, what):
+    """Every y and h_last element against the oracle at BASELINE.json's per-element bound."""
+    yref, hlref = ref
     y, hl = gpu_selective(inp, variant)
-    assert torch.isfinite(y.float()).all() and torch.isfinite(hl).all()
-    yref, hlref = oracle_selective_rows(inp, rows)
-    bi = torch.tensor([r[0] for r in rows], device=y.device)
-    di = torch.tensor([r[1] for r in rows], device=y.device)
-    assert_close(y[bi, di], yref, dtype, f"{what} y")
-    assert_close(hl[bi, di], hlref, dtype, f"{what} h_last")
-    return y, hl
+    assert y.numel() == yref.size and hl.numel() == hlref.size
+    e1 = assert_close_all(y, yref, dtype, f"{what} y")
+    e2 = assert_close_all(hl, hlref, dtype, f"{what} h_last")
+    return e1, e2
 
 
-def test_config3_selective_bf16_mamba_scale_sampled_rows(cuda_device):
-    """Full size, in the launch configuration bench.py times (AUTO), on sampled rows the
-    oracle computes one by one; plus both forced variants."""
+def test_config3_selective_bf16_mamba_scale_every_element(cuda_device):
+    """Full size (batch 8 x d_inner 4096 x L 2048 = 67 108 864 outputs), in the launch
+    configuration bench.py times (AUTO -> lane_row), every element against the oracle; then
+    every other schedule that accepts the shape, also on every element."""
     c = config(3)
     inp = make_selective_inputs(c, device=cuda_device)
-    rows = _sample_rows(c.batch, c.d_inner, 96, 3)
-    y, hl = _check_selective_sampled(inp, lib.VARIANT_AUTO, rows, c.dtype, "cfg3 auto")
+    ref = oracle_selective_all_rows(inp)
+    assert ref[0].size == c.batch * c.d_inner * c.L
+    _check_selective_every_element(inp, ref, lib.VARIANT_AUTO, c.dtype, "cfg3 auto")
     assert lib.last_variant() == lib.SELECTIVE_LANE_ROW
-    y2, hl2 = _check_selective_sampled(inp, lib.SELECTIVE_WARP_ROW, rows, c.dtype, "cfg3 warp_row")
-    # the two schedules agree everywhere (not only on the sampled rows) to bf16 rounding
-    # (lane_row evaluates a share of its 2^x with the degree-3 polynomial for bf16 io: 4.3e-4)
-    assert rel_err(hl2, to_f64_numpy(hl)) <= 2e-3
-    assert (y.float() - y2.float()).abs().max().item() <= 2e-2 * (1 + y.float().abs().max().item())
+    for v in (lib.SELECTIVE_WARP_ROW, lib.SELECTIVE_WARP_ROW_TMA):
+        _check_selective_every_element(inp, ref, v, c.dtype, f"cfg3 {lib.VARIANT_NAMES[v]}")
 
 
-def test_config4_selective_long_sequence_sampled_rows(cuda_device):
+def test_config4_selective_long_sequence_every_element(cuda_device):
+    """batch 1 x d_inner 1536 x L 65536 = 100 663 296 outputs, every element, every schedule."""
     c = config(4)
     inp = make_selective_inputs(c, device=cuda_device)
-    rows = _sample_rows(c.batch, c.d_inner, 24, 4)
-    _check_selective_sampled(inp, lib.VARIANT_AUTO, rows, c.dtype, "cfg4 auto")
-    assert lib.last_variant() == lib.SELECTIVE_WARP_ROW_TMA
-    _check_selective_sampled(inp, lib.SELECTIVE_WARP_ROW, rows, c.dtype, "cfg4 warp_row")
-    _check_selective_sampled(inp, lib.SELECTIVE_LANE_ROW, rows, c.dtype, "cfg4 lane_row")
+    ref = oracle_selective_all_rows(inp, rows_per_task=8)
+    assert ref[0].size == c.batch * c.d_inner * c.L
+    _check_selective_every_element(inp, ref, lib.VARIANT_AUTO, c.dtype, "cfg4 auto")
+    auto = lib.last_variant()
+    assert auto in FEW_ROWS_VARIANTS
+    for v in SELECTIVE_VARIANTS:
+        if v != auto:
+            _check_selective_every_element(inp, ref, v, c.dtype, f"cfg4 {lib.VARIANT_NAMES[v]}")
 
 
-def test_config5_affine_bandwidth_sweep_sampled_sequences(cuda_device):
-    """2^30 elements re-segmented into L = 2^10 .. 2^20.  Sampled sequences against the oracle;
-    every element against the recurrence itself (a property that holds at any size)."""
+def test_config5_affine_bandwidth_sweep_every_element(cuda_device):
+    """2^30 elements re-segmented into L = 2^10 .. 2^20.  ALL 2^30 outputs of each of the six
+    lengths are compared with the oracle, streamed slab by slab (2^24 elements, whole sequences)
+    so no 8 GB float64 array is materialised; the slabs run on several host
+    threads.  Also the forced look-back schedule on the longest and one short length."""
+    from concurrent.futures import ThreadPoolExecutor
     total = 1 << 30
+    slab = 1 << 24
     flat = make_affine_inputs(config(5, L=total, total=total), device=cuda_device)
     a_flat, u_flat = flat["a"].reshape(-1), flat["u"].reshape(-1)
     h0_all = normal((1 << 20,), seed=config(5).seed, stream=3, device=cuda_device,
                     dtype=torch.float32)
-    h = torch.empty(total, dtype=torch.float32, device=cuda_device)
-    rng = np.random.default_rng(5)
-    for logL in (10, 12, 14, 16, 18, 20):
+    runs = [(logL, lib.VARIANT_AUTO) for logL in (10, 12, 14, 16, 18, 20)]
+    runs += [(20, lib.AFFINE_LOOKBACK), (12, lib.AFFINE_LOOKBACK)]
+    outs = []
+    for logL, variant in runs:
         L = 1 << logL
         S = total // L
-        a, u, h0 = a_flat.view(S, L), u_flat.view(S, L), h0_all[:S]
-        hv = h.view(S, L)
-        hl = torch.empty(S, dtype=torch.float32, device=cuda_device)
-        lib.affine_scan(a, u, h0, hv, hl)
+        h = torch.full((S, L), float("nan"), dtype=torch.float32, device=cuda_device)
+        hl = torch.full((S,), float("nan"), dtype=torch.float32, device=cuda_device)
+        lib.affine_scan_ex(a_flat.view(S, L), u_flat.view(S, L), h0_all[:S], h, hl, variant)
         torch.cuda.synchronize()
-        # AUTO: long sequences, enough of them => one CTA each; many short ones => one warp each
-        assert lib.last_variant() == (lib.AFFINE_CTA_LOOP if L >= 8192 else lib.AFFINE_WARP_SEQ)
-        # sampled sequences, element by element
-        seqs = sorted({0, S - 1, *[int(v) for v in rng.integers(S, size=8 if L >= 1 << 18 else 32)]})
-        idx = torch.tensor(seqs, device=cuda_device)
-        href, hlref = oracle.affine_scan(to_f64_numpy(a[idx]), to_f64_numpy(u[idx]),
-                                         to_f64_numpy(h0[idx]))
-        assert_close(hv[idx], href, torch.float32, f"cfg5 L=2^{logL} h")
-        assert_close(hl[idx], hlref, torch.float32, f"cfg5 L=2^{logL} h_last")
-        # all elements: h_last is the last column; the recurrence holds step by step
-        assert torch.equal(hl, hv[:, -1])
-        worst = 0.0
-        for s0 in range(0, S, max(1, (1 << 26) // L)):
-            s1 = min(S, s0 + max(1, (1 << 26) // L))
-            hb = hv[s0:s1].double()
-            prev = torch.cat([h0[s0:s1].double()[:, None], hb[:, :-1]], dim=1)
-            res = (hb - (a[s0:s1].double() * prev + u[s0:s1].double())).abs() / (1 + hb.abs())
-            worst = max(worst, res.max().item())
-        assert worst <= 1e-5, f"cfg5 L=2^{logL}: recurrence residual {worst:.2e}"
+        if variant == lib.VARIANT_AUTO:
+            # long sequences, enough of them => one CTA each; many short ones => one warp each
+            assert lib.last_variant() == (lib.AFFINE_CTA_LOOP if L >= 8192 else lib.AFFINE_WARP_SEQ)
+        outs.append((L, S, variant, h, hl))
+    h0_host = h0_all.double().cpu().numpy()
+
+    def check_slab(i):
+        s0, s1 = i * slab, (i + 1) * slab
+        a64 = a_flat[s0:s1].double().cpu().numpy()
+        u64 = u_flat[s0:s1].double().cpu().numpy()
+        worst = {}
+        for (L, S, variant, h, hl) in outs:
+            q0, q1 = s0 // L, s1 // L                    # whole sequences: slab % L == 0
+            href, hlref = oracle.affine_scan(a64.reshape(-1, L), u64.reshape(-1, L), h0_host[q0:q1])
+            e = rel_err_device(h[q0:q1], href)
+            e2 = rel_err_device(hl[q0:q1], hlref)
+            worst[(L, variant)] = max(e, e2)
+        return worst
+
+    compared = 0
+    with ThreadPoolExecutor(min(8, host_threads())) as pool:
+        for worst in pool.map(check_slab, range(total // slab)):
+            compared += slab
+            for (L, variant), e in worst.items():
+                assert e <= TOL[torch.float32], \
+                    f"cfg5 L={L} variant {variant}: max|err|/(1+|ref|) = {e:.3e}"
+    assert compared == total
 
 
 # ============================================================ seeded random shapes (fuzz)

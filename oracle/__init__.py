@@ -10,5 +10,7 @@ from .oracle import (  # noqa: F401
     build,
     compose,
     fold_pairs,
+    selective_scan_bwd,
     selective_scan_fwd,
+    selective_scan_fwd_ext,
 )

@@ -45,6 +45,10 @@ def _load():
         lib.oracle_affine_scan.restype = None
         lib.oracle_selective_scan_fwd.argtypes = [_dp] * 9 + [_i64] * 4
         lib.oracle_selective_scan_fwd.restype = None
+        lib.oracle_selective_scan_fwd_ext.argtypes = [_dp] * 12 + [_i64] * 5
+        lib.oracle_selective_scan_fwd_ext.restype = None
+        lib.oracle_selective_scan_bwd.argtypes = [_dp] * 16 + [_i64] * 4
+        lib.oracle_selective_scan_bwd.restype = None
         lib.oracle_compose.argtypes = [ctypes.c_double] * 4 + [_dp, _dp]
         lib.oracle_compose.restype = None
         lib.oracle_fold_pairs.argtypes = [_dp, _dp, _i64, _dp, _dp]
@@ -111,6 +115,68 @@ def selective_scan_fwd(x, delta, A, B, C, D=None, h0=None):
     _load().oracle_selective_scan_fwd(_ptr(x), _ptr(delta), _ptr(A), _ptr(B), _ptr(C), _ptr(D),
                                       _ptr(h0), _ptr(y), _ptr(h_last), batch, d_inner, N, L)
     return y, h_last
+
+
+def selective_scan_fwd_ext(x, delta, A, B, C, D=None, z=None, delta_bias=None, reset=None,
+                           h0=None, delta_softplus=False):
+    """Forward selective scan with the fused steps either side of the recurrence (PAPER.md
+    §6.7, §9): Delta = softplus(delta + delta_bias[d]) if ``delta_softplus`` (else delta +
+    bias), state reset to 0 where ``reset[b, t] != 0``, and y <- y * silu(z).
+
+    z: [batch, d_inner, L] or None; delta_bias: [d_inner] or None; reset: [batch, L] or None.
+    Returns (y, h_last) in float64.
+    """
+    x = _f64(x)
+    if x.ndim != 3:
+        raise ValueError("oracle.selective_scan_fwd_ext: x must be [batch, d_inner, L]")
+    batch, d_inner, L = x.shape
+    delta = _f64(delta, (batch, d_inner, L))
+    A = _f64(A)
+    if A.ndim != 2 or A.shape[0] != d_inner:
+        raise ValueError("oracle.selective_scan_fwd_ext: A must be [d_inner, N]")
+    N = A.shape[1]
+    B = _f64(B, (batch, N, L))
+    C = _f64(C, (batch, N, L))
+    D = _f64(D, (d_inner,))
+    z = _f64(z, (batch, d_inner, L))
+    delta_bias = _f64(delta_bias, (d_inner,))
+    reset = _f64(reset, (batch, L))
+    h0 = _f64(h0, (batch, d_inner, N))
+    y = np.empty((batch, d_inner, L), dtype=np.float64)
+    h_last = np.empty((batch, d_inner, N), dtype=np.float64)
+    _load().oracle_selective_scan_fwd_ext(_ptr(x), _ptr(delta), _ptr(A), _ptr(B), _ptr(C),
+                                          _ptr(D), _ptr(z), _ptr(delta_bias), _ptr(reset),
+                                          _ptr(h0), _ptr(y), _ptr(h_last), batch, d_inner, N, L,
+                                          1 if delta_softplus else 0)
+    return y, h_last
+
+
+def selective_scan_bwd(x, delta, A, B, C, D, h0, dy, dh_last=None):
+    """Gradients of loss = <dy, y> + <dh_last, h_last> of ``selective_scan_fwd`` with respect
+    to every input.  Returns dict(dx, ddelta, dA, dB, dC, dD, dh0) in float64."""
+    x = _f64(x)
+    batch, d_inner, L = x.shape
+    delta = _f64(delta, (batch, d_inner, L))
+    A = _f64(A)
+    N = A.shape[1]
+    B = _f64(B, (batch, N, L))
+    C = _f64(C, (batch, N, L))
+    D = _f64(D, (d_inner,))
+    h0 = _f64(h0, (batch, d_inner, N))
+    dy = _f64(dy, (batch, d_inner, L))
+    dh_last = _f64(dh_last, (batch, d_inner, N))
+    out = {
+        "dx": np.empty((batch, d_inner, L)), "ddelta": np.empty((batch, d_inner, L)),
+        "dA": np.empty((d_inner, N)), "dB": np.empty((batch, N, L)),
+        "dC": np.empty((batch, N, L)), "dD": np.empty((d_inner,)),
+        "dh0": np.empty((batch, d_inner, N)),
+    }
+    _load().oracle_selective_scan_bwd(_ptr(x), _ptr(delta), _ptr(A), _ptr(B), _ptr(C), _ptr(D),
+                                      _ptr(h0), _ptr(dy), _ptr(dh_last), _ptr(out["dx"]),
+                                      _ptr(out["ddelta"]), _ptr(out["dA"]), _ptr(out["dB"]),
+                                      _ptr(out["dC"]), _ptr(out["dD"]), _ptr(out["dh0"]),
+                                      batch, d_inner, N, L)
+    return out
 
 
 def compose(later, earlier):

@@ -18,14 +18,23 @@
  *     void*; NULL = the legacy default stream): they enqueue work and return without
  *     synchronising.  `_host` entry points synchronise `cuda_stream` before returning.
  *   - The library owns only a small per-(device, stream) scratch for the decoupled
- *     look-back tile descriptors, grown on demand and freed at unload.
+ *     look-back tile descriptors.  It is allocated, grown and cleared IN STREAM ORDER on
+ *     `cuda_stream` (cudaMallocAsync / cudaFreeAsync / cudaMemsetAsync): no device entry
+ *     point synchronises the host or the device, and none clears the scratch per call
+ *     (descriptor statuses carry a per-launch epoch).  Device entry points may be captured
+ *     in a CUDA graph: inside a capture the scratch is a per-call stream-ordered
+ *     allocation owned by the graph.  A captured graph must not run concurrently with
+ *     itself.  Calls on different streams may run concurrently from different threads.
  *   - Errors are integer status codes (affinescan_status); nothing aborts, throws or
  *     prints.  Misaligned pointers or an L that is not a multiple of the 128-bit
  *     vector width are NOT errors: a scalar-load kernel is chosen.
  *   - State and accumulation are fp32; io dtype is fp32 or bf16; outputs are rounded
  *     to the io dtype with round-to-nearest-even; h_last is always fp32.
  *   - Results are bitwise reproducible run to run for a given variant (values are
- *     never accumulated with atomics).
+ *     never accumulated with atomics), except AFFINESCAN_AFFINE_LOOKBACK and
+ *     AFFINESCAN_SELECTIVE_CHUNKED, whose decoupled look-back folds whichever predecessor
+ *     aggregates are published at poll time: reproducible up to the floating-point
+ *     association order of P:90 Eq.(7) (all orders are within the stated tolerance).
  */
 #ifndef AFFINESCAN_H_
 #define AFFINESCAN_H_
@@ -82,10 +91,27 @@ typedef enum affinescan_variant {
                                                sharing B_t/C_t tiles staged in shared memory
                                                by TMA tensor copies (needs N == 16, 16-byte
                                                aligned pointers, L a multiple of the vector) */
-    AFFINESCAN_SELECTIVE_LANE_ROW = 12  /* one lane per (b,d) row, sequential in L, x/Δ/y
-                                           and B/C tiles staged in shared memory by TMA
-                                           bulk copies (needs d_inner % 32 == 0)          */
+    AFFINESCAN_SELECTIVE_LANE_ROW = 12, /* one lane per (b,d) row, sequential in L; B/C tiles
+                                           staged in shared memory by TMA tensor copies
+                                           (needs N == 16, d_inner % 32 == 0, 16-byte aligned
+                                           pointers, L a multiple of the vector)           */
+    AFFINESCAN_SELECTIVE_CHUNKED = 14   /* few rows x long L: L is cut into chunks that run on
+                                           different CTAs; the carry h_in crosses chunks by
+                                           decoupled look-back over per-(row, state) chunk
+                                           aggregates (BJ "decoupled look-back for very long
+                                           sequences"; same shape requirements as WARP_ROW_TMA) */
 } affinescan_variant;
+
+/* Structure the caller asserts about A: a hint the
+ * library may exploit; the result is what the general kernel computes on the same A. */
+typedef enum affinescan_a_structure {
+    AFFINESCAN_A_GENERAL = 0,        /* any A[d,n]                                          */
+    AFFINESCAN_A_SCALAR_PER_ROW = 1, /* A[d,n] == A[d,0] for every n (one decay per row):
+                                        one exp per (b,d,t) instead of N                    */
+    AFFINESCAN_A_POWERS = 2          /* A[d,n] == (n+1)*A[d,0] (S4D-real structure):
+                                        a_n = r^(n+1), r = exp(delta*A[d,0]): one exp and
+                                        N-1 multiplies per (b,d,t)                          */
+} affinescan_a_structure;
 
 /* ------------------------------------------------------------------------------------
  * affine_scan — inclusive scan of the affine recurrence
@@ -166,6 +192,65 @@ AFFINESCAN_API int selective_scan_fwd_host(const void* x, const void* delta, con
                                            int io_dtype, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------
+ * selective_scan_fwd_ext — selective_scan_fwd with the steps either side of the scan that a
+ * production selective-scan kernel fuses beyond the affine recurrence ("integrates
+ * recurrence, projection, and gating") and the reset mechanism the paper leaves
+ * unmodelled.  Every extra pointer may be NULL (=> that step is absent); with all of
+ * them NULL and delta_softplus == 0 this is selective_scan_fwd_ex.
+ *
+ *     Delta_t[d] = softplus(delta_t[d] + delta_bias[d])    if delta_softplus != 0
+ *                = delta_t[d] + delta_bias[d]              otherwise
+ *     reset[b,t] != 0  =>  step t starts a new sequence: h_{t-1} := 0, i.e. the transition
+ *                          pair of step t is (0, u_t), a left zero of (+) (Eq.7); with
+ *                          reset[b,0] != 0 the initial state h0 of that batch is ignored.
+ *                          Packs several variable-length sequences along L.
+ *     a_t, u_t, h_t, y_t as in selective_scan_fwd with Delta_t
+ *     y_t[d] <- y_t[d] * silu(z_t[d]),   silu(v) = v / (1 + exp(-v))          if z != NULL
+ *
+ *   z           [batch, d_inner, L]  io dtype   in, NULL => no gate
+ *   delta_bias  [d_inner]            fp32       in, NULL => 0
+ *   reset       [batch, L]           uint8      in, NULL => no resets
+ *   a_structure an affinescan_a_structure the caller asserts about A (0 = general)
+ *   variant     AFFINESCAN_VARIANT_AUTO or an AFFINESCAN_SELECTIVE_*
+ * softplus is evaluated as log2(1 + 2^(v log2 e)) ln 2 with MUFU.EX2 / MUFU.LG2 (v > 20: v;
+ * small 2^..: its series), silu with MUFU.EX2 / MUFU.RCP.
+ * ------------------------------------------------------------------------------------ */
+AFFINESCAN_API int selective_scan_fwd_ext(const void* x, const void* delta, const float* A,
+                                          const void* B, const void* C, const float* D,
+                                          const void* z, const float* delta_bias,
+                                          const uint8_t* reset, const float* h0, void* y,
+                                          float* h_last, int batch, int d_inner, int N,
+                                          int64_t L, int io_dtype, int delta_softplus,
+                                          int a_structure, int variant, void* cuda_stream);
+
+/* Same computation with HOST buffers (see selective_scan_fwd_host). */
+AFFINESCAN_API int selective_scan_fwd_ext_host(const void* x, const void* delta, const float* A,
+                                               const void* B, const void* C, const float* D,
+                                               const void* z, const float* delta_bias,
+                                               const uint8_t* reset, const float* h0, void* y,
+                                               float* h_last, int batch, int d_inner, int N,
+                                               int64_t L, int io_dtype, int delta_softplus,
+                                               int a_structure, void* cuda_stream);
+
+/* The gated form of a Mamba block: Delta = softplus(delta_raw + delta_bias[d])
+ * as a prologue and y <- y * silu(z) as an epilogue of the same kernel (no extra pass over
+ * HBM).  delta_bias and z may be NULL.  Equals selective_scan_fwd_ext(..., reset = NULL,
+ * delta_softplus = 1, AFFINESCAN_A_GENERAL, AFFINESCAN_VARIANT_AUTO). */
+AFFINESCAN_API int selective_scan_fwd_gated(const void* x, const void* delta_raw,
+                                            const float* delta_bias, const float* A,
+                                            const void* B, const void* C, const float* D,
+                                            const void* z, const float* h0, void* y,
+                                            float* h_last, int batch, int d_inner, int N,
+                                            int64_t L, int io_dtype, void* cuda_stream);
+
+/* reset[t] = 1 where a packed sequence starts (t = cu_seqlens[i], i = 0..num_seq-1; entries
+ * outside [0, L) are ignored), 0 elsewhere.  cu_seqlens: [num_seq] int32, device; reset: [L]
+ * uint8, device (one batch row of selective_scan_fwd_ext's reset).  Asynchronous on the stream. */
+AFFINESCAN_API int affinescan_reset_mask_from_cu_seqlens(const int32_t* cu_seqlens, int num_seq,
+                                                         uint8_t* reset, int64_t L,
+                                                         void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
  * Introspection (no device work)
  * ------------------------------------------------------------------------------------ */
 /* Static, NUL-terminated description of a status code. */
@@ -182,12 +267,13 @@ AFFINESCAN_API int affinescan_version(void);
 /* Tuning knobs for ablations and sweeps (process-wide; -1 restores the default chosen from
  * the shape).  Returns AFFINESCAN_ERR_UNSUPPORTED for an unknown key or value. */
 typedef enum affinescan_option {
-    AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lanes per (b,d) row in the lane_row schedule: 1, 2, 4 */
-    AFFINESCAN_OPT_LANE_ROW_POLY16 = 2  /* sixteenths (0, 3..6) of the exponentials evaluated by
+    AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lanes per (b,d) row in the lane_row schedule: 1, 2   */
+    AFFINESCAN_OPT_LANE_ROW_POLY16 = 2  /* sixteenths (0 or 4) of the exponentials evaluated by
                                            the fma-pipe polynomial instead of MUFU.EX2           */
 } affinescan_option;
 AFFINESCAN_API int affinescan_set_option(int key, int value);
-/* Frees the cached scratch / staging buffers of the current device (synchronises it). */
+/* Frees the cached scratch / staging buffers, copy streams and events of the current device
+ * (synchronises it).  Must not run concurrently with other calls into the library. */
 AFFINESCAN_API int affinescan_release_cache(void);
 
 #ifdef __cplusplus

@@ -26,12 +26,17 @@ AFFINE_WARP_SEQ = 4
 SELECTIVE_WARP_ROW = 11
 SELECTIVE_LANE_ROW = 12
 SELECTIVE_WARP_ROW_TMA = 13
+SELECTIVE_CHUNKED = 14
+
+A_GENERAL = 0
+A_SCALAR_PER_ROW = 1
+A_POWERS = 2
 
 VARIANT_NAMES = {
     0: "auto", 1: "affine_lookback", 2: "affine_cta_loop", 3: "affine_blelloch",
     4: "affine_warp_seq",
     11: "selective_warp_row", 12: "selective_lane_row",
-    13: "selective_warp_row_tma",
+    13: "selective_warp_row_tma", 14: "selective_chunked",
 }
 
 _vp = ctypes.c_void_p
@@ -45,6 +50,10 @@ _SIGNATURES = {
     "selective_scan_fwd": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _vp]),
     "selective_scan_fwd_ex": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _int, _vp]),
     "selective_scan_fwd_host": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _vp]),
+    "selective_scan_fwd_ext": (_int, [_vp] * 12 + [_int, _int, _int, _i64, _int, _int, _int, _int, _vp]),
+    "selective_scan_fwd_ext_host": (_int, [_vp] * 12 + [_int, _int, _int, _i64, _int, _int, _int, _vp]),
+    "selective_scan_fwd_gated": (_int, [_vp] * 11 + [_int, _int, _int, _i64, _int, _vp]),
+    "affinescan_reset_mask_from_cu_seqlens": (_int, [_vp, _int, _vp, _i64, _vp]),
     "affinescan_status_string": (ctypes.c_char_p, [_int]),
     "affinescan_last_cuda_error": (_int, []),
     "affinescan_last_variant": (_int, []),
@@ -219,6 +228,58 @@ def selective_scan_fwd_host(x, delta, A, B, C, D, h0, y, h_last, stream=None):
     args = _selective_args(x, delta, A, B, C, D, h0, y, h_last, "cpu")
     _check("selective_scan_fwd_host",
            load().selective_scan_fwd_host(*args, _stream_ptr(stream, x)))
+
+
+def _ext_args(x, delta, A, B, C, D, z, delta_bias, reset, h0, y, h_last, device):
+    base = _selective_args(x, delta, A, B, C, D, h0, y, h_last, device)
+    batch, d_inner, L = x.shape
+    (px, pdelta, pA, pB, pC, pD, ph0, py, phl, batch, d_inner, N, L, io) = base
+    return (px, pdelta, pA, pB, pC, pD,
+            _ptr(z, dtype=x.dtype, shape=(batch, d_inner, L), device=device, name="z"),
+            _ptr(delta_bias, dtype=torch.float32, shape=(d_inner,), device=device, name="delta_bias"),
+            _ptr(reset, dtype=torch.uint8, shape=(batch, L), device=device, name="reset"),
+            ph0, py, phl, batch, d_inner, N, L, io)
+
+
+def selective_scan_fwd_ext(x, delta, A, B, C, D, z, delta_bias, reset, h0, y, h_last,
+                           delta_softplus=False, a_structure=A_GENERAL, variant=VARIANT_AUTO,
+                           stream=None):
+    """selective_scan_fwd with the fused softplus/bias prologue, silu(z) gate and resets."""
+    args = _ext_args(x, delta, A, B, C, D, z, delta_bias, reset, h0, y, h_last, "cuda")
+    with torch.cuda.device(x.device):
+        _check("selective_scan_fwd_ext",
+               load().selective_scan_fwd_ext(*args, int(bool(delta_softplus)), int(a_structure),
+                                             int(variant), _stream_ptr(stream, x)))
+
+
+def selective_scan_fwd_ext_host(x, delta, A, B, C, D, z, delta_bias, reset, h0, y, h_last,
+                                delta_softplus=False, a_structure=A_GENERAL, stream=None):
+    args = _ext_args(x, delta, A, B, C, D, z, delta_bias, reset, h0, y, h_last, "cpu")
+    _check("selective_scan_fwd_ext_host",
+           load().selective_scan_fwd_ext_host(*args, int(bool(delta_softplus)), int(a_structure),
+                                              _stream_ptr(stream, x)))
+
+
+def selective_scan_fwd_gated(x, delta_raw, delta_bias, A, B, C, D, z, h0, y, h_last, stream=None):
+    """Delta = softplus(delta_raw + delta_bias[d]) prologue and y * silu(z) epilogue, fused."""
+    (px, pdelta, pA, pB, pC, pD, pz, pbias, _, ph0, py, phl, batch, d_inner, N, L, io) = _ext_args(
+        x, delta_raw, A, B, C, D, z, delta_bias, None, h0, y, h_last, "cuda")
+    with torch.cuda.device(x.device):
+        _check("selective_scan_fwd_gated",
+               load().selective_scan_fwd_gated(px, pdelta, pbias, pA, pB, pC, pD, pz, ph0, py, phl,
+                                               batch, d_inner, N, L, io, _stream_ptr(stream, x)))
+
+
+def reset_mask_from_cu_seqlens(cu_seqlens, reset_row, stream=None):
+    """reset_row[t] = 1 at every t in cu_seqlens (int32, device), 0 elsewhere; reset_row: [L] uint8."""
+    if cu_seqlens.dtype != torch.int32 or reset_row.dtype != torch.uint8:
+        raise TypeError("cu_seqlens must be int32 and reset_row uint8")
+    with torch.cuda.device(reset_row.device):
+        _check("affinescan_reset_mask_from_cu_seqlens",
+               load().affinescan_reset_mask_from_cu_seqlens(
+                   _ptr(cu_seqlens, device="cuda", name="cu_seqlens"), int(cu_seqlens.numel()),
+                   _ptr(reset_row, device="cuda", name="reset_row"), int(reset_row.numel()),
+                   _stream_ptr(stream, reset_row)))
 
 
 # ------------------------------------------------------------------------ introspection

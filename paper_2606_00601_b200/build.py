@@ -13,12 +13,16 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG_DIR)
 CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libaffinescan.so")
-SOURCES = [os.path.join(CSRC, "affinescan_api.cu")]
-NVCC_FLAGS = [
+SOURCES = [os.path.join(CSRC, n) for n in
+           ("affinescan_api.cu", "affinescan_affine.cu", "affinescan_selective.cu")]
+NVCC_COMPILE_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",
-    "-cudart", "static",
-    "-shared", "-Xcompiler", "-fPIC,-fvisibility=hidden",
+    "-Xcompiler", "-fPIC,-fvisibility=hidden",
+]
+NVCC_LINK_FLAGS = [
+    "-gencode", "arch=compute_100a,code=sm_100a",
+    "-cudart", "static", "-shared", "-Xcompiler", "-fPIC,-fvisibility=hidden",
 ]
 
 
@@ -48,14 +52,28 @@ def build(force: bool = False, verbose: bool = False) -> str:
     """Compile the CUDA extension if it is missing or older than its sources."""
     if not force and not is_stale():
         return LIB_PATH
-    tmp = LIB_PATH + f".tmp{os.getpid()}"
-    cmd = [_nvcc(), *NVCC_FLAGS, "-I", os.path.join(ROOT, "include"), "-o", tmp, *SOURCES]
-    if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
-        print(" ".join(cmd), file=sys.stderr)
-    subprocess.check_call(cmd)
-    os.replace(tmp, LIB_PATH)
+    from concurrent.futures import ThreadPoolExecutor
+    nvcc = _nvcc()
+    objdir = os.path.join(PKG_DIR, "build", f"obj{os.getpid()}")
+    os.makedirs(objdir, exist_ok=True)
+
+    def compile_one(src):
+        obj = os.path.join(objdir, os.path.basename(src) + ".o")
+        cmd = [nvcc, *NVCC_COMPILE_FLAGS, "-I", os.path.join(ROOT, "include"), "-c", "-o", obj, src]
+        if verbose:
+            cmd[1:1] = ["-Xptxas", "-v"]
+            print(" ".join(cmd), file=sys.stderr)
+        subprocess.check_call(cmd)
+        return obj
+
+    try:
+        with ThreadPoolExecutor(len(SOURCES)) as pool:   # one nvcc per translation unit
+            objs = list(pool.map(compile_one, SOURCES))
+        tmp = LIB_PATH + f".tmp{os.getpid()}"
+        subprocess.check_call([nvcc, *NVCC_LINK_FLAGS, "-o", tmp, *objs])
+        os.replace(tmp, LIB_PATH)
+    finally:
+        shutil.rmtree(objdir, ignore_errors=True)
     return LIB_PATH
 
 

@@ -18,22 +18,35 @@ namespace affinescan {
 // ------------------------------------------------------------------ tile descriptors
 // One descriptor per tile = two 64-bit words {status:32 | float bits:32}: word 0 carries
 // P, word 1 carries U.  Each word is written with ONE 64-bit store, so a reader that
-// sees equal non-empty statuses in both words holds a consistent pair.  INCLUSIVE
+// sees equal valid statuses in both words holds a consistent pair.  INCLUSIVE
 // descriptors carry (0, h_end): the state after the tile, as a left-zero pair.
+// status = (tag << 2) | state with tag = the launch's epoch + 1 (never 0): words left by an
+// earlier launch, or the zero fill of a fresh buffer, read as EMPTY, so the descriptors are
+// never cleared between calls.  The control block holds the tile ticket, the count of finished
+// tiles and the epoch; the last tile to finish resets the first two and bumps the epoch, which
+// also makes a captured CUDA graph replayable.
 constexpr unsigned kDescEmpty = 0u;
 constexpr unsigned kDescAggregate = 1u;
 constexpr unsigned kDescInclusive = 2u;
 
-__device__ __forceinline__ void desc_store(unsigned long long* d, unsigned status, Pair v)
+struct LookbackCtrl {
+    unsigned ticket;
+    unsigned done;
+    unsigned epoch;
+    unsigned pad;
+};
+
+__device__ __forceinline__ void desc_store(unsigned long long* d, unsigned tag, unsigned state,
+                                           Pair v)
 {
-    const unsigned long long hi = static_cast<unsigned long long>(status) << 32;
+    const unsigned long long hi = static_cast<unsigned long long>((tag << 2) | state) << 32;
     const unsigned long long w0 = hi | __float_as_uint(v.P);
     const unsigned long long w1 = hi | __float_as_uint(v.U);
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(d), "l"(w0) : "memory");
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(d + 1), "l"(w1) : "memory");
 }
 
-__device__ __forceinline__ unsigned desc_load(const unsigned long long* d, Pair& v)
+__device__ __forceinline__ unsigned desc_load(const unsigned long long* d, unsigned tag, Pair& v)
 {
     unsigned long long w0, w1;
     asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(w0) : "l"(d) : "memory");
@@ -42,7 +55,8 @@ __device__ __forceinline__ unsigned desc_load(const unsigned long long* d, Pair&
     const unsigned s1 = static_cast<unsigned>(w1 >> 32);
     v.P = __uint_as_float(static_cast<unsigned>(w0));
     v.U = __uint_as_float(static_cast<unsigned>(w1));
-    return s0 == s1 ? s0 : kDescEmpty;  // torn read (mid-transition) => retry
+    // another epoch's word, or a torn read (mid-transition) => EMPTY: retry
+    return (s0 == s1 && (s0 >> 2) == (tag & 0x3fffffffu)) ? (s0 & 3u) : kDescEmpty;
 }
 
 // ------------------------------------------------------------------ per-thread tile state
@@ -108,13 +122,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32))
 affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
                             const float* __restrict__ h0, T* __restrict__ h,
                             float* __restrict__ h_last, long long total, long long L,
-                            unsigned long long* __restrict__ desc, unsigned* __restrict__ ticket)
+                            unsigned long long* __restrict__ desc, LookbackCtrl* __restrict__ ctrl)
 {
     constexpr int kWarpElems = 32 * VEC * J;
     constexpr int kTile = WARPS * kWarpElems;
     using Acc = Access<T, VEC, true>;
 
-    __shared__ unsigned s_tile;
+    __shared__ unsigned s_tile, s_tag;
     __shared__ long long s_q0, s_r0;
     __shared__ Pair s_warp[WARPS];
     __shared__ float s_hin;
@@ -125,14 +139,16 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
     // Tile ids come from a ticket so that every predecessor tile is already running
     // when its successor looks back (forward progress without relying on block order).
     if (threadIdx.x == 0) {
-        const unsigned tk = atomicAdd(ticket, 1u);
+        const unsigned tk = atomicAdd(&ctrl->ticket, 1u);
         const long long b = static_cast<long long>(tk) * kTile;
         s_tile = tk;
+        s_tag = (*reinterpret_cast<volatile unsigned*>(&ctrl->epoch) + 1u) & 0x3fffffffu;
         s_q0 = b / L;
         s_r0 = b % L;
     }
     __syncthreads();
     const unsigned tile = s_tile;
+    const unsigned tag = s_tag;
     const long long base = static_cast<long long>(tile) * kTile;
     const long long q0 = s_q0, r0 = s_r0;
 
@@ -178,8 +194,8 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
         const bool need_carry = (r0 != 0);  // a tile that starts at a head ignores its carry-in
         const bool self_contained = (agg.P == 0.0f) || !need_carry;
         if (lane == 0) {
-            if (self_contained) desc_store(my, kDescInclusive, Pair{0.0f, agg.U});
-            else desc_store(my, kDescAggregate, agg);
+            if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, agg.U});
+            else desc_store(my, tag, kDescAggregate, agg);
         }
         float h_in = 0.0f;
         if (need_carry) {
@@ -191,10 +207,10 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
                 unsigned st = kDescInclusive;  // before the stream: state 0
                 if (idx >= 0) {
                     const unsigned long long* d = desc + 2ull * idx;
-                    st = desc_load(d, e);
+                    st = desc_load(d, tag, e);
                     while (st == kDescEmpty) {  // back off: the poll competes with the data stream
                         __nanosleep(64);
-                        st = desc_load(d, e);
+                        st = desc_load(d, tag, e);
                     }
                 }
                 __syncwarp();
@@ -214,7 +230,7 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
             }
             h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
             if (lane == 0 && !self_contained)
-                desc_store(my, kDescInclusive, Pair{0.0f, apply(agg, h_in)});
+                desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(agg, h_in)});
         }
         if (lane == 0) s_hin = h_in;
     }
@@ -241,6 +257,19 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
             }
         }
         H = apply(r.tot[j], H);
+    }
+    // The last tile to finish re-arms the control block for the next launch on this buffer.
+    // Every other tile has published its INCLUSIVE descriptor before it counts itself done
+    // (the barrier above orders warp 0's store before thread 0's atomic).
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned ntiles = gridDim.x;
+        if (atomicAdd(&ctrl->done, 1u) == ntiles - 1) {
+            ctrl->ticket = 0;
+            ctrl->done = 0;
+            ctrl->epoch = tag;  // = old epoch + 1 (mod 2^30)
+            __threadfence();
+        }
     }
 }
 

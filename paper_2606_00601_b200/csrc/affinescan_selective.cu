@@ -1,0 +1,419 @@
+// affinescan_selective.cu — host launch layer of selective_scan_fwd and its extended forms
+// (include/affinescan.h): validates, picks a kernel variant from the shape, encodes (and caches)
+// the TMA tensor maps of B and C, and enqueues ONE kernel on the caller's stream.
+#include <atomic>
+#include <limits>
+#include <map>
+#include <mutex>
+#include <tuple>
+
+#include "host_internal.h"
+#include "selective_scan_lane_row.cuh"
+#include "selective_scan_warp_row.cuh"
+#include "selective_scan_warp_row_tma.cuh"
+
+namespace affinescan_host {
+
+using namespace affinescan;
+using bf16 = __nv_bfloat16;
+
+namespace {
+
+constexpr int kWarpRowTmaMaxWarps = 11;   // warp_row_tma: rows per CTA (+1 producer warp = 384 threads)
+constexpr int64_t kWarpRowTmaMinL = 1024; // below two warp tiles the plain warp_row is as good
+constexpr int64_t kChunkedMinL = 8192;    // chunked (look-back) schedule: at least ~10 tiles per row
+constexpr int kSelWarps = 4;        // warp_row: rows per CTA
+constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
+constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
+constexpr int kLaneRowDefaultG = 1;       // lanes per row (r01b sweep: profiles/)
+constexpr int kLaneRowDefaultPoly16 = 4;  // sixteenths of the exps done on the fma pipe
+
+// Tuning knobs of the lane_row schedule (affinescan_set_option); -1 = choose from the shape.
+std::atomic<int> g_opt_lane_row_g{-1};
+std::atomic<int> g_opt_lane_row_poly16{-1};
+
+// ---------------------------------------------------------------- TMA tensor maps
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda).
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                   const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                   const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+int get_encode_tiled(EncodeTiledFn* out)
+{
+    static std::atomic<void*> cached{nullptr};
+    void* fn = cached.load(std::memory_order_acquire);
+    if (!fn) {
+        cudaDriverEntryPointQueryResult qres;
+        AS_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (qres != cudaDriverEntryPointSuccess || !fn) return cuda_fail(cudaErrorNotSupported);
+        cached.store(fn, std::memory_order_release);
+    }
+    *out = reinterpret_cast<EncodeTiledFn>(fn);
+    return AFFINESCAN_OK;
+}
+
+// Tensor map over a [rows = batch*N, L] io-dtype matrix (B or C), box = {box_t timesteps, N rows}.
+// A map depends only on (pointer, shape, box, dtype), so it is encoded once and cached: repeated
+// calls on the same tensors (a training loop, a replayed graph) pay a map lookup, not a driver
+// call.  The cache is bounded; it is dropped when full.
+struct MapKey {
+    const void* base;
+    int64_t rows, L;
+    int box_t, N, esize;
+    bool operator<(const MapKey& o) const
+    {
+        return std::tie(base, rows, L, box_t, N, esize) <
+               std::tie(o.base, o.rows, o.L, o.box_t, o.N, o.esize);
+    }
+};
+std::mutex g_map_mu;
+std::map<MapKey, CUtensorMap> g_maps;
+constexpr size_t kMaxCachedMaps = 512;
+
+template <typename T>
+int make_bc_tensor_map(CUtensorMap* map, const T* base, int64_t rows, int64_t L, int box_t, int N)
+{
+    const MapKey key{base, rows, L, box_t, N, static_cast<int>(sizeof(T))};
+    {
+        std::lock_guard<std::mutex> lk(g_map_mu);
+        auto it = g_maps.find(key);
+        if (it != g_maps.end()) {
+            *map = it->second;
+            return AFFINESCAN_OK;
+        }
+    }
+    EncodeTiledFn encode = nullptr;
+    AS_TRY(get_encode_tiled(&encode));
+    const cuuint64_t dims[2] = {static_cast<cuuint64_t>(L), static_cast<cuuint64_t>(rows)};
+    const cuuint64_t strides[1] = {static_cast<cuuint64_t>(L) * sizeof(T)};
+    const cuuint32_t box[2] = {static_cast<cuuint32_t>(box_t), static_cast<cuuint32_t>(N)};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(map, sizeof(T) == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
+                                                  : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
+                              2, const_cast<T*>(base), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return cuda_fail(cudaErrorInvalidValue);
+    std::lock_guard<std::mutex> lk(g_map_mu);
+    if (g_maps.size() >= kMaxCachedMaps) g_maps.clear();
+    g_maps[key] = *map;
+    return AFFINESCAN_OK;
+}
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (kernel, device).  Keyed by the
+// kernel's address: instantiations share one function-pointer TYPE, so a static per template
+// instantiation of this helper would be shared by all of them.
+std::mutex g_attr_mu;
+std::map<std::pair<const void*, int>, int> g_attr_done;
+
+template <typename Kern>
+int allow_smem(Kern kern, int bytes)
+{
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    const std::pair<const void*, int> key{reinterpret_cast<const void*>(kern), dev};
+    std::lock_guard<std::mutex> lk(g_attr_mu);
+    auto it = g_attr_done.find(key);
+    if (it == g_attr_done.end() || it->second < bytes) {
+        AS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        g_attr_done[key] = bytes;
+    }
+    return AFFINESCAN_OK;
+}
+
+// ---------------------------------------------------------------- typed view of the arguments
+template <typename T>
+struct Typed {
+    const T *x, *delta, *B, *C;
+    T* y;
+    const float *A, *D, *h0;
+    float* h_last;
+    SelectiveExt ext;
+    bool has_ext;
+    int batch, d_inner, N;
+    int64_t L;
+};
+
+template <typename T>
+Typed<T> typed(const SelectiveArgs& a)
+{
+    Typed<T> t;
+    t.x = static_cast<const T*>(a.x);
+    t.delta = static_cast<const T*>(a.delta);
+    t.B = static_cast<const T*>(a.B);
+    t.C = static_cast<const T*>(a.C);
+    t.y = static_cast<T*>(a.y);
+    t.A = a.A;
+    t.D = a.D;
+    t.h0 = a.h0;
+    t.h_last = a.h_last;
+    t.ext = SelectiveExt{a.z, a.delta_bias, a.reset, a.delta_softplus};
+    t.has_ext = a.z || a.delta_bias || a.reset || a.delta_softplus;
+    t.batch = a.batch;
+    t.d_inner = a.d_inner;
+    t.N = a.N;
+    t.L = a.L;
+    return t;
+}
+
+// ---------------------------------------------------------------- warp_row (general fallback)
+template <typename T, int VEC, int NV, bool EXT>
+int launch_warp_row_inst(const Typed<T>& t, cudaStream_t stream)
+{
+    const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
+    const int64_t blocks = (rows + kSelWarps - 1) / kSelWarps;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    selective_scan_warp_row_kernel<T, VEC, NV, kSelWarps, EXT>
+        <<<static_cast<unsigned>(blocks), kSelWarps * 32, 0, stream>>>(
+            t.x, t.delta, t.A, t.B, t.C, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner, t.N,
+            t.L);
+    return after_launch();
+}
+
+template <typename T>
+int launch_warp_row(const Typed<T>& t, bool vec_ok, cudaStream_t stream)
+{
+    constexpr int kVec = Io<T>::kVec;
+    if (vec_ok)
+        return t.has_ext ? launch_warp_row_inst<T, kVec, 16 / kVec, true>(t, stream)
+                         : launch_warp_row_inst<T, kVec, 16 / kVec, false>(t, stream);
+    return t.has_ext ? launch_warp_row_inst<T, 1, 4, true>(t, stream)
+                     : launch_warp_row_inst<T, 1, 4, false>(t, stream);
+}
+
+// ---------------------------------------------------------------- lane_row (many rows)
+template <typename T, int G, int F16, bool EXT, int ASTR>
+int launch_lane_row_inst(const Typed<T>& t, cudaStream_t stream)
+{
+    // polynomial degree per io dtype: DESIGN.md §7 (tolerance argument)
+    constexpr int kDeg = sizeof(T) == 2 ? 3 : 5;
+    using S = LaneRowSmem<T, kLaneRowTc>;
+    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg, EXT, ASTR>;
+    constexpr int smem = S::kPerWarp * kLaneRowWarps;
+    AS_TRY(allow_smem(kern, smem));
+    CUtensorMap mapB, mapC;
+    AS_TRY(make_bc_tensor_map<T>(&mapB, t.B, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
+    AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
+    const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
+    const int64_t warps = rows / (32 / G);
+    const int64_t blocks = (warps + kLaneRowWarps - 1) / kLaneRowWarps;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    kern<<<static_cast<unsigned>(blocks), kLaneRowWarps * 32, smem, stream>>>(
+        t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner, t.L);
+    return after_launch();
+}
+
+template <typename T, int G, int F16>
+int launch_lane_row_gf(const Typed<T>& t, cudaStream_t stream)
+{
+    return t.has_ext ? launch_lane_row_inst<T, G, F16, true, 0>(t, stream)
+                     : launch_lane_row_inst<T, G, F16, false, 0>(t, stream);
+}
+
+template <typename T>
+int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
+{
+    if (a_structure == AFFINESCAN_A_SCALAR_PER_ROW)
+        return t.has_ext ? launch_lane_row_inst<T, 1, 0, true, 1>(t, stream)
+                         : launch_lane_row_inst<T, 1, 0, false, 1>(t, stream);
+    if (a_structure == AFFINESCAN_A_POWERS)
+        return t.has_ext ? launch_lane_row_inst<T, 1, 0, true, 2>(t, stream)
+                         : launch_lane_row_inst<T, 1, 0, false, 2>(t, stream);
+    int G = g_opt_lane_row_g.load(std::memory_order_relaxed);
+    int poly16 = g_opt_lane_row_poly16.load(std::memory_order_relaxed);
+    if (G < 0) G = kLaneRowDefaultG;
+    if (poly16 < 0) poly16 = kLaneRowDefaultPoly16;
+    if (G == 1 && poly16 == 0) return launch_lane_row_gf<T, 1, 0>(t, stream);
+    if (G == 1 && poly16 == 4) return launch_lane_row_gf<T, 1, 4>(t, stream);
+    if (G == 2 && poly16 == 0) return launch_lane_row_gf<T, 2, 0>(t, stream);
+    if (G == 2 && poly16 == 4) return launch_lane_row_gf<T, 2, 4>(t, stream);
+    return AFFINESCAN_ERR_UNSUPPORTED;
+}
+
+// ---------------------------------------------------------------- warp_row_tma (few rows)
+constexpr int kScratchSlotChunked = 1;
+
+template <typename T>
+struct TmaShape {
+    static constexpr int kVec = Io<T>::kVec;
+    // odd: conflict-free LDS.128 (K = 12 fp32 / 24 bf16 timesteps per lane; K = 20 with one
+    // chain measured slower: cfg4 0.906 vs 0.818 ms)
+    static constexpr int kNv = 3;
+    // fp32 io: two states per n-iteration (two independent chains); bf16 io: K = 24 leaves
+    // registers for one chain only.
+    static constexpr int kNu = sizeof(T) == 2 ? 1 : 2;
+    using S = WarpRowTmaSmem<T, kNv * kVec>;
+};
+
+// CHUNKED: persistent CTAs draw (tile, row-block) items tile-major; carry by decoupled look-back
+template <typename T, bool EXT>
+int launch_chunked_inst(const Typed<T>& t, cudaStream_t stream)
+{
+    using Sh = TmaShape<T>;
+    using S = typename Sh::S;
+    auto kern = selective_scan_warp_row_tma_kernel<T, Sh::kVec, Sh::kNv, Sh::kNu, EXT, true>;
+    AS_TRY(allow_smem(kern, S::kBytes));
+    CUtensorMap mapB, mapC;
+    AS_TRY(make_bc_tensor_map<T>(&mapB, t.B, static_cast<int64_t>(t.batch) * 16, t.L, S::kBoxT, 16));
+    AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, S::kBoxT, 16));
+    int sms = 0;
+    AS_TRY(sm_count(&sms));
+    const int R = t.d_inner < kWarpRowTmaMaxWarps ? t.d_inner : kWarpRowTmaMaxWarps;
+    const int ctas_per_batch = (t.d_inner + R - 1) / R;
+    const int64_t ntiles = (t.L + S::kTileT - 1) / S::kTileT;
+    int64_t nitems = 0, ndesc = 0;
+    const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
+    if (mul_overflows(ntiles, static_cast<int64_t>(t.batch) * ctas_per_batch, &nitems) ||
+        nitems > 0x7ffffff0LL || mul_overflows(rows * 16, ntiles, &ndesc) ||
+        ndesc > (std::numeric_limits<int64_t>::max() >> 5))
+        return AFFINESCAN_ERR_UNSUPPORTED;
+    // [LookbackCtrl | rows x ntiles x N descriptors of 16 B]; zero-filled when fresh, never
+    // cleared afterwards (epoch-tagged statuses)
+    Scratch sc;
+    AS_TRY(scratch_acquire(stream, kScratchSlotChunked,
+                           sizeof(LookbackCtrl) + static_cast<size_t>(ndesc) * 16, &sc));
+    auto* ctrl = static_cast<LookbackCtrl*>(sc.ptr);
+    auto* desc = reinterpret_cast<unsigned long long*>(ctrl + 1);
+    const int64_t grid = nitems < sms ? nitems : sms;  // one persistent CTA per SM
+    kern<<<static_cast<unsigned>(grid), (R + 1) * 32, S::kBytes, stream>>>(
+        t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner,
+        ctas_per_batch, t.L, desc, ctrl);
+    const int st = after_launch();
+    const int st2 = scratch_release(stream, sc);
+    return st != AFFINESCAN_OK ? st : st2;
+}
+
+template <typename T>
+int launch_chunked(const Typed<T>& t, cudaStream_t stream)
+{
+    return t.has_ext ? launch_chunked_inst<T, true>(t, stream)
+                     : launch_chunked_inst<T, false>(t, stream);
+}
+
+template <typename T, bool EXT>
+int launch_warp_row_tma_inst(const Typed<T>& t, cudaStream_t stream)
+{
+    using Sh = TmaShape<T>;
+    using S = typename Sh::S;
+    auto kern = selective_scan_warp_row_tma_kernel<T, Sh::kVec, Sh::kNv, Sh::kNu, EXT, false>;
+    AS_TRY(allow_smem(kern, S::kBytes));
+    CUtensorMap mapB, mapC;
+    AS_TRY(make_bc_tensor_map<T>(&mapB, t.B, static_cast<int64_t>(t.batch) * 16, t.L, S::kBoxT, 16));
+    AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, S::kBoxT, 16));
+    // R rows (warps) of one batch per CTA, sized so that one wave of CTAs covers all rows when
+    // they fit (cfg2/cfg4 on 148 SMs: 1536 rows -> 140 CTAs of 11 warps)
+    int sms = 0;
+    AS_TRY(sm_count(&sms));
+    const int slots = sms / t.batch > 0 ? sms / t.batch : 1;
+    int R = (t.d_inner + slots - 1) / slots;  // consumer warps per CTA
+    R = R < 1 ? 1 : (R > kWarpRowTmaMaxWarps ? kWarpRowTmaMaxWarps : R);
+    const int ctas_per_batch = (t.d_inner + R - 1) / R;
+    const int64_t blocks = static_cast<int64_t>(t.batch) * ctas_per_batch;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    kern<<<static_cast<unsigned>(blocks), (R + 1) * 32, S::kBytes, stream>>>(
+        t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner,
+        ctas_per_batch, t.L, nullptr, nullptr);
+    return after_launch();
+}
+
+template <typename T>
+int launch_warp_row_tma(const Typed<T>& t, cudaStream_t stream)
+{
+    return t.has_ext ? launch_warp_row_tma_inst<T, true>(t, stream)
+                     : launch_warp_row_tma_inst<T, false>(t, stream);
+}
+
+// ---------------------------------------------------------------- dispatch
+template <typename T>
+int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
+{
+    const Typed<T> t = typed<T>(a);
+    constexpr int kVec = Io<T>::kVec;
+    const bool vec_ok = (t.L % kVec == 0) && aligned16(t.x) && aligned16(t.delta) &&
+                        aligned16(t.B) && aligned16(t.C) && aligned16(t.y) &&
+                        (!a.z || aligned16(a.z));
+    const bool lane_ok_common = vec_ok && t.L < (1LL << 31) - 4096;  // TMA coordinates are int32
+    const bool lane_ok = lane_ok_common && t.N == 16 && (t.d_inner % 32 == 0) && aligned16(t.A) &&
+                         (!t.h0 || aligned16(t.h0)) && (!t.h_last || aligned16(t.h_last));
+    const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
+    const bool tma_ok = lane_ok_common && t.N == 16;
+    int variant = a.variant;
+    if (variant == AFFINESCAN_VARIANT_AUTO) {
+        int sms = 0;
+        AS_TRY(sm_count(&sms));
+        // one row per FP32 lane of the machine; the structured-A paths need far
+        // fewer instructions per row-step, so they pay off from one warp per sub-partition
+        const int64_t lane_row_min_rows = static_cast<int64_t>(sms) * 128;
+        // too few rows to give every SM a CTA of row-warps, and at least a few tiles per row:
+        // parallelise L across CTAs with the decoupled look-back carry
+        const bool few_rows = rows * 2 < static_cast<int64_t>(sms) * kWarpRowTmaMaxWarps;
+        if (lane_ok && rows >= lane_row_min_rows) variant = AFFINESCAN_SELECTIVE_LANE_ROW;
+        else if (tma_ok && few_rows && t.L >= kChunkedMinL) variant = AFFINESCAN_SELECTIVE_CHUNKED;
+        else if (tma_ok && t.L >= kWarpRowTmaMinL) variant = AFFINESCAN_SELECTIVE_WARP_ROW_TMA;
+        else variant = AFFINESCAN_SELECTIVE_WARP_ROW;
+    }
+    int st;
+    switch (variant) {
+    case AFFINESCAN_SELECTIVE_WARP_ROW:
+        st = launch_warp_row<T>(t, vec_ok, stream);
+        break;
+    case AFFINESCAN_SELECTIVE_WARP_ROW_TMA:
+        if (!tma_ok) return AFFINESCAN_ERR_UNSUPPORTED;
+        st = launch_warp_row_tma<T>(t, stream);
+        break;
+    case AFFINESCAN_SELECTIVE_CHUNKED:
+        if (!tma_ok) return AFFINESCAN_ERR_UNSUPPORTED;
+        st = launch_chunked<T>(t, stream);
+        break;
+    case AFFINESCAN_SELECTIVE_LANE_ROW:
+        if (!lane_ok) return AFFINESCAN_ERR_UNSUPPORTED;
+        st = launch_lane_row<T>(t, a.a_structure, stream);
+        break;
+    default:
+        return AFFINESCAN_ERR_UNSUPPORTED;
+    }
+    if (st == AFFINESCAN_OK) set_last_variant(variant);
+    return st;
+}
+
+}  // namespace
+
+int set_lane_row_option(int key, int value)
+{
+    switch (key) {
+    case AFFINESCAN_OPT_LANE_ROW_G:
+        if (value != -1 && value != 1 && value != 2) return AFFINESCAN_ERR_UNSUPPORTED;
+        g_opt_lane_row_g.store(value);
+        return AFFINESCAN_OK;
+    case AFFINESCAN_OPT_LANE_ROW_POLY16:
+        if (value != -1 && value != 0 && value != 4) return AFFINESCAN_ERR_UNSUPPORTED;
+        g_opt_lane_row_poly16.store(value);
+        return AFFINESCAN_OK;
+    default: return AFFINESCAN_ERR_UNSUPPORTED;
+    }
+}
+
+int selective_scan_impl(const SelectiveArgs& a, void* cuda_stream)
+{
+    set_last_variant(0);
+    if (a.io_dtype != AFFINESCAN_F32 && a.io_dtype != AFFINESCAN_BF16) return AFFINESCAN_ERR_DTYPE;
+    if (a.batch < 0 || a.d_inner < 0 || a.L < 0) return AFFINESCAN_ERR_SHAPE;
+    if (a.N < 1 || a.N > AFFINESCAN_MAX_N) return AFFINESCAN_ERR_UNSUPPORTED;
+    if (a.a_structure < AFFINESCAN_A_GENERAL || a.a_structure > AFFINESCAN_A_POWERS)
+        return AFFINESCAN_ERR_UNSUPPORTED;
+    int64_t rows = 0, total = 0, bnl = 0;
+    if (mul_overflows(a.batch, a.d_inner, &rows) || mul_overflows(rows, a.L, &total) ||
+        mul_overflows(static_cast<int64_t>(a.batch) * a.N, a.L, &bnl) ||
+        total > (std::numeric_limits<int64_t>::max() >> 3) ||
+        bnl > (std::numeric_limits<int64_t>::max() >> 3))
+        return AFFINESCAN_ERR_SHAPE;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    if (rows == 0) return AFFINESCAN_OK;
+    if (a.L == 0) return fill_h_last(a.h0, a.h_last, rows * a.N, stream);
+    if (!a.x || !a.delta || !a.A || !a.B || !a.C || !a.y) return AFFINESCAN_ERR_NULL;
+    return a.io_dtype == AFFINESCAN_F32 ? selective_dispatch<float>(a, stream)
+                                        : selective_dispatch<bf16>(a, stream);
+}
+
+}  // namespace affinescan_host

@@ -1,175 +1,42 @@
 // selective_scan_lane_row.cuh — variant AFFINESCAN_SELECTIVE_LANE_ROW of
 // selective_scan_fwd (include/affinescan.h; BJ north_star).
 //
-// G lanes share one (b,d) row (G = 1, 2 or 4); each lane keeps NS = 16/G of the row's N = 16
-// states h[n] and A2[n] = A[d,n]*log2(e) in registers, packed two states per 64-bit register
-// pair, and walks L sequentially: no warp scan, no rescan.  Per pair of state-steps the work is
-//     arg  = {delta,delta} * A2pair          FMUL2   (fma-pipe, mul.rn.f32x2)
+// The many-rows schedule (cfg3).  G lanes share one (b,d) row (G = 1, 2 or 4); each lane keeps
+// NS = 16/G of the row's N = 16 states h[n] and A2[n] = A[d,n]*log2(e) in registers, packed two
+// states per 64-bit register pair, and walks L sequentially: no warp scan, no rescan.  Per pair
+// of state-steps the work is
+//     arg  = {delta,delta} * A2pair          FMUL2   (fma pipe, mul.rn.f32x2)
 //     a    = 2^arg                           2 x MUFU.EX2   -- or, for a compile-time share of the
 //                                            (timestep, pair) slots, a Cody-Waite + minimax
 //                                            polynomial 2^x evaluated with FFMA2 on the fma pipe
 //     u    = {delta*x,delta*x} * Bpair       FMUL2
 //     h    = a*h + u                         FFMA2   (Eq.3 with the pair of P:86 Eq.6)
 //     y   += Cpair*h                         FFMA2   (BJ: y = sum_n C h + D x; h never stored)
+// issued "pass-major": one pass = four states over the VEC timesteps of a 128-bit group, first
+// every 2^x of the pass, then the dependent h chains.
 // A warp covers 32/G consecutive d of one batch b, so B_t/C_t are warp-uniform: each warp stages
 // its [2][N][TC] B/C tile with two TMA tensor copies per tile (cp.async.bulk.tensor.2d through
-// tensor maps over [batch*N, L], mbarrier complete_tx, double-buffered; SASS UTMALDG), transposes/widens it once to an fp32 [TC][2][N] tile, and every
-// state-step then reads B/C with broadcast LDS.128.  x/delta come from global memory as raw
-// 128-bit words prefetched two groups ahead; y is reduced across the G lanes of the row with a
-// shuffle reduce-scatter and leaves with 128/G-bit stores.  Warps are autonomous: no CTA barrier.
+// tensor maps over [batch*N, L], mbarrier complete_tx, double-buffered; SASS UTMALDG),
+// transposes/widens it once to an fp32 [TC][2][N] tile, and every state-step then reads B/C with
+// broadcast LDS.128.  x/delta come from global memory as raw 128-bit words prefetched two groups
+// ahead; y is reduced across the G lanes of the row with a shuffle reduce-scatter and leaves
+// with 128/G-bit stores.  Warps are autonomous: no CTA barrier.
+//
+// Template options:
+//   EXT   the fused steps either side of the scan: Delta = softplus(delta +
+//         bias[d]), y <- y*silu(z), resets (the pair of a reset step is the left zero (0, u_t)).
+//   ASTR  structured-A fast paths (P:118-122 generality): 0 = general A;
+//         1 = one decay per row, A[d,n] = A[d,0] (one 2^x per (b,d,t));
+//         2 = A[d,n] = (n+1) A[d,0]: a_n = r^(n+1), r = 2^(delta A2[d,0]) (one 2^x and a chain of
+//             packed multiplies per (b,d,t)).
 #pragma once
 
 #include <type_traits>
 
-#include <cuda.h>  // CUtensorMap (type only; the encoder is fetched through the runtime)
-
-#include "common.cuh"
+#include "selective_common.cuh"
+#include "tma.cuh"
 
 namespace affinescan {
-
-// ------------------------------------------------------------------ mbarrier / TMA bulk copy
-__device__ __forceinline__ uint32_t smem_u32(const void* p)
-{
-    return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count)
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
-                 "r"(bytes)
-                 : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, unsigned parity)
-{
-    unsigned ok;
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity)
-{
-    while (!mbar_try_wait(bar, parity)) {}
-}
-// TMA 1-D bulk copy global -> shared, completion reported to an mbarrier (SASS: UBLKCP).
-__device__ __forceinline__ void tma_bulk_g2s(void* dst_smem, const void* src_gmem, unsigned bytes,
-                                             uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-        ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
-        : "memory");
-}
-// TMA 2-D tiled copy global -> shared through a tensor map: box {TC timesteps, N rows} at
-// element coordinates (c0 = t, c1 = row); out-of-range elements are zero-filled and still
-// counted in complete_tx (SASS: UTMALDG).
-__device__ __forceinline__ void tma_tile_2d_g2s(void* dst_smem, const CUtensorMap* map, int c0,
-                                                int c1, uint64_t* bar)
-{
-    asm volatile(
-        "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes "
-        "[%0], [%1, {%2, %3}], [%4];"
-        ::"r"(smem_u32(dst_smem)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
-        : "memory");
-}
-__device__ __forceinline__ void fence_proxy_async_smem()
-{
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-}
-__device__ __forceinline__ void fence_mbar_init()
-{
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-
-// ------------------------------------------------------------------ packed fp32x2 arithmetic
-// A "pair" is two fp32 values in one 64-bit register pair; SASS: FFMA2 / FMUL2 / FADD2.
-using pair_t = unsigned long long;
-
-__device__ __forceinline__ pair_t pk(float lo, float hi)
-{
-    pair_t r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void upk(pair_t v, float& lo, float& hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ pair_t fma2(pair_t a, pair_t b, pair_t c)
-{
-    pair_t d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ pair_t mul2(pair_t a, pair_t b)
-{
-    pair_t d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-
-// ------------------------------------------------------------------ 2^x on the fma pipe
-// x = i + r, i = round(x), r in [-1/2, 1/2];  2^x = 2^i * p(r),  p(r) = 1 + r*q(r) with q the
-// minimax approximation of (2^r - 1)/r (error measured relative to 2^r - 1, so that a = 2^x close
-// to 1 keeps an accurate 1 - a: DESIGN.md §7).  Valid for |x| <= 126 (the caller clamps delta).
-template <int DEG>
-struct Exp2Coef;
-template <>
-struct Exp2Coef<3> {  // max |p - 2^r| / |2^r - 1| = 4.3e-4
-    static __device__ __forceinline__ float c(int i)
-    {
-        constexpr float k[3] = {6.931782961e-01f, 2.420288622e-01f, 5.550396442e-02f};
-        return k[i];
-    }
-};
-template <>
-struct Exp2Coef<4> {  // 1.5e-5
-    static __device__ __forceinline__ float c(int i)
-    {
-        constexpr float k[4] = {6.931368709e-01f, 2.402325273e-01f, 5.583728850e-02f,
-                                9.618110955e-03f};
-        return k[i];
-    }
-};
-template <>
-struct Exp2Coef<5> {  // 4.3e-7 (then fp32 rounding)
-    static __device__ __forceinline__ float c(int i)
-    {
-        constexpr float k[5] = {6.931471229e-01f, 2.402235121e-01f, 5.550500378e-02f,
-                                9.666245431e-03f, 1.333353925e-03f};
-        return k[i];
-    }
-};
-
-// {2^(d*A2.lo), 2^(d*A2.hi)} for dd = {d,d}: 3 + DEG FFMA2 and two integer adds.
-template <int DEG>
-__device__ __forceinline__ pair_t exp2_poly2(pair_t dd, pair_t A2p)
-{
-    constexpr float kMagic = 12582912.0f;  // 1.5 * 2^23: fma rounds x to the nearest integer
-    const pair_t magic = pk(kMagic, kMagic);
-    const pair_t t = fma2(dd, A2p, magic);                   // bits(t) = 0x4B400000 + i
-    const pair_t ni = fma2(t, pk(-1.0f, -1.0f), magic);      // -i, exact
-    const pair_t r = fma2(dd, A2p, ni);                      // x - i with one rounding
-    pair_t q = pk(Exp2Coef<DEG>::c(DEG - 1), Exp2Coef<DEG>::c(DEG - 1));
-#pragma unroll
-    for (int j = DEG - 2; j >= 0; --j) q = fma2(q, r, pk(Exp2Coef<DEG>::c(j), Exp2Coef<DEG>::c(j)));
-    const pair_t p = fma2(q, r, pk(1.0f, 1.0f));
-    float plo, phi, tlo, thi;
-    upk(p, plo, phi);
-    upk(t, tlo, thi);
-    // 2^i by adding i to the exponent field: (bits(t) << 23) == i << 23 (mod 2^32)
-    const float alo = __uint_as_float(__float_as_uint(plo) + (__float_as_uint(tlo) << 23));
-    const float ahi = __uint_as_float(__float_as_uint(phi) + (__float_as_uint(thi) << 23));
-    return pk(alo, ahi);
-}
 
 // Which (timestep-in-group k, pair p) slots use the polynomial: F16 of every 16 slots, spread
 // evenly (Bresenham), decided at compile time.
@@ -189,49 +56,83 @@ struct LaneRowSmem {
     static_assert(kRawStage % 256 == 0 && kPerWarp % 128 == 0, "TMA destinations: 128 B aligned");
 };
 
-// y elements per lane after the reduce-scatter: io-dtype store of CNT consecutive values.
+// CNT consecutive io-dtype values at p <-> floats (16 / 8 / 4 / 2-byte accesses).
 template <typename T, int CNT>
-__device__ __forceinline__ void store_y(T* p, const float (&v)[CNT]);
+struct RowSeg;
 template <>
-__device__ __forceinline__ void store_y<float, 4>(float* p, const float (&v)[4])
-{
-    __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
-}
+struct RowSeg<float, 4> {
+    static __device__ __forceinline__ void store(float* p, const float (&v)[4])
+    {
+        __stcs(reinterpret_cast<float4*>(p), make_float4(v[0], v[1], v[2], v[3]));
+    }
+    static __device__ __forceinline__ void load(const float* p, float (&v)[4])
+    {
+        const float4 r = __ldcs(reinterpret_cast<const float4*>(p));
+        v[0] = r.x; v[1] = r.y; v[2] = r.z; v[3] = r.w;
+    }
+};
 template <>
-__device__ __forceinline__ void store_y<float, 2>(float* p, const float (&v)[2])
-{
-    __stcs(reinterpret_cast<float2*>(p), make_float2(v[0], v[1]));
-}
+struct RowSeg<float, 2> {
+    static __device__ __forceinline__ void store(float* p, const float (&v)[2])
+    {
+        __stcs(reinterpret_cast<float2*>(p), make_float2(v[0], v[1]));
+    }
+    static __device__ __forceinline__ void load(const float* p, float (&v)[2])
+    {
+        const float2 r = __ldcs(reinterpret_cast<const float2*>(p));
+        v[0] = r.x; v[1] = r.y;
+    }
+};
 template <>
-__device__ __forceinline__ void store_y<float, 1>(float* p, const float (&v)[1])
-{
-    __stcs(p, v[0]);
-}
+struct RowSeg<float, 1> {
+    static __device__ __forceinline__ void store(float* p, const float (&v)[1]) { __stcs(p, v[0]); }
+    static __device__ __forceinline__ void load(const float* p, float (&v)[1]) { v[0] = __ldcs(p); }
+};
 template <>
-__device__ __forceinline__ void store_y<__nv_bfloat16, 8>(__nv_bfloat16* p, const float (&v)[8])
-{
-    __stcs(reinterpret_cast<uint4*>(p),
-           make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]), pack_bf16x2(v[4], v[5]),
-                      pack_bf16x2(v[6], v[7])));
-}
+struct RowSeg<__nv_bfloat16, 8> {
+    static __device__ __forceinline__ void store(__nv_bfloat16* p, const float (&v)[8])
+    {
+        __stcs(reinterpret_cast<uint4*>(p),
+               make_uint4(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3]),
+                          pack_bf16x2(v[4], v[5]), pack_bf16x2(v[6], v[7])));
+    }
+    static __device__ __forceinline__ void load(const __nv_bfloat16* p, float (&v)[8])
+    {
+        unpack128<__nv_bfloat16>(__ldcs(reinterpret_cast<const uint4*>(p)), v);
+    }
+};
 template <>
-__device__ __forceinline__ void store_y<__nv_bfloat16, 4>(__nv_bfloat16* p, const float (&v)[4])
-{
-    __stcs(reinterpret_cast<uint2*>(p),
-           make_uint2(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3])));
-}
+struct RowSeg<__nv_bfloat16, 4> {
+    static __device__ __forceinline__ void store(__nv_bfloat16* p, const float (&v)[4])
+    {
+        __stcs(reinterpret_cast<uint2*>(p),
+               make_uint2(pack_bf16x2(v[0], v[1]), pack_bf16x2(v[2], v[3])));
+    }
+    static __device__ __forceinline__ void load(const __nv_bfloat16* p, float (&v)[4])
+    {
+        const uint2 r = __ldcs(reinterpret_cast<const uint2*>(p));
+        v[0] = bf16_lo(r.x); v[1] = bf16_hi(r.x); v[2] = bf16_lo(r.y); v[3] = bf16_hi(r.y);
+    }
+};
 template <>
-__device__ __forceinline__ void store_y<__nv_bfloat16, 2>(__nv_bfloat16* p, const float (&v)[2])
-{
-    __stcs(reinterpret_cast<unsigned*>(p), pack_bf16x2(v[0], v[1]));
-}
+struct RowSeg<__nv_bfloat16, 2> {
+    static __device__ __forceinline__ void store(__nv_bfloat16* p, const float (&v)[2])
+    {
+        __stcs(reinterpret_cast<unsigned*>(p), pack_bf16x2(v[0], v[1]));
+    }
+    static __device__ __forceinline__ void load(const __nv_bfloat16* p, float (&v)[2])
+    {
+        const unsigned r = __ldcs(reinterpret_cast<const unsigned*>(p));
+        v[0] = bf16_lo(r); v[1] = bf16_hi(r);
+    }
+};
 
 // ====================================================================================
 // The kernel.  T = io dtype; G = lanes per row; TC = timesteps per staged B/C tile;
 // WARPS = warps per CTA; F16 = sixteenths of the exponentials done by the polynomial;
-// DEG = its degree; PP = packed pairs per pass (2*PP states share one MUFU burst).
+// DEG = its degree; EXT / ASTR: see the header comment.
 // ====================================================================================
-template <typename T, int G, int TC, int WARPS, int F16, int DEG, int PP, bool PIPE>
+template <typename T, int G, int TC, int WARPS, int F16, int DEG, bool EXT, int ASTR>
 __global__ void __launch_bounds__(WARPS * 32)
 selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                const float* __restrict__ A,
@@ -239,7 +140,8 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                                const __grid_constant__ CUtensorMap mapC,
                                const float* __restrict__ D,
                                const float* __restrict__ h0, T* __restrict__ y,
-                               float* __restrict__ h_last, int batch, int d_inner, long long L)
+                               float* __restrict__ h_last, const SelectiveExt ext, int batch,
+                               int d_inner, long long L)
 {
     using S = LaneRowSmem<T, TC>;
     constexpr int N = S::N;
@@ -248,10 +150,12 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     constexpr int RW = 32 / G;         // rows per warp
     constexpr int NS = N / G;          // states per lane
     constexpr int NP = NS / 2;         // packed pairs per lane
+    constexpr int PP = 2;              // packed pairs per pass (four states share a MUFU burst)
     constexpr int YC = VEC / G;        // y values per lane after the reduce-scatter
     static_assert(G == 1 || G == 2 || G == 4, "G");
-    static_assert(PP % 2 == 0 && (N / G / 2) % PP == 0, "pairs per pass");
+    static_assert(NP % PP == 0, "pairs per pass");
     static_assert(NS % 4 == 0 && YC >= 1 && TC % VEC == 0 && (TC / VEC) % 2 == 0, "shape");
+    static_assert(ASTR == 0 || (G == 1 && F16 == 0), "structured-A paths: one lane per row, no polynomial");
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
@@ -307,13 +211,19 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
         h2[2 * q + 0] = pk(hv.x, hv.y);
         h2[2 * q + 1] = pk(hv.z, hv.w);
     }
+    float A20 = 0.0f;  // structured-A paths read A[d,0] only
+    if (ASTR != 0) A20 = __ldg(A + static_cast<long long>(d) * N) * kLog2e;
     // the polynomial is used only while |delta*A2| <= 126 for every state of the lane
     const float dmax = 126.0f / (amax * kLog2e);
     const float Dg = (D && g == 0) ? __ldg(D + d) : 0.0f;  // the skip term is added by one lane
+    const float bias = (EXT && ext.delta_bias) ? __ldg(ext.delta_bias + d) : 0.0f;
 
     const T* xr = x + row * L;
     const T* dr = delta + row * L;
     T* yr = y + row * L;
+    const T* zr = EXT ? static_cast<const T*>(ext.z) : nullptr;
+    if (EXT && zr) zr += row * L;
+    const unsigned char* rst = (EXT && ext.reset) ? ext.reset + static_cast<long long>(b) * L : nullptr;
     // timestep offset, inside a VEC group, of the YC values this lane stores
     int yoff = 0;
     if (G >= 2) yoff += (g & (G / 2)) ? VEC / 2 : 0;
@@ -369,12 +279,23 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         xq[pi] = __ldcs(reinterpret_cast<const uint4*>(xr + tg + PD * VEC));
                         dq[pi] = __ldcs(reinterpret_cast<const uint4*>(dr + tg + PD * VEC));
                     }
+                    // f1 prologue: Delta = softplus(delta + bias[d]); f2: reset bits of the group
+                    unsigned rmask = 0;
+                    float zv[YC];
+                    if (EXT) {
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            dl[k] += bias;
+                            if (ext.delta_softplus) dl[k] = softplus_f(dl[k]);
+                        }
+                        if (rst) {
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k)
+                                rmask |= (__ldg(rst + tg + k) != 0 ? 1u : 0u) << k;
+                        }
+                        if (zr) RowSeg<T, YC>::load(zr + tg + yoff, zv);
+                    }
                     float ys[VEC];
-                    // One pass = four states (two packed pairs, one LDS.128 of B and of C per
-                    // timestep) over the VEC timesteps of the group: first every 2^x of the pass
-                    // (independent: they stream through the MUFU / fma pipes back to back), then
-                    // the two dependent h chains.  F = sixteenths of the exps taken by the
-                    // polynomial (0 on the guarded slow path).
                     float dxs[VEC];
                     pair_t y2[VEC];
 #pragma unroll
@@ -382,8 +303,27 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         dxs[k] = dl[k] * xv[k];
                         y2[k] = pk(Dg * xv[k], 0.0f);
                     }
-                    auto pass = [&](int q, auto ftag) {  // pairs [PP*q, PP*q + PP)
+                    // structured A: the decay base r_k = 2^(delta_k A2[d,0]) of each timestep
+                    pair_t cur[ASTR == 2 ? VEC : 1];
+                    float r1[ASTR != 0 ? VEC : 1], r2[ASTR == 2 ? VEC : 1];
+                    if (ASTR != 0) {
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            r1[k] = ex2_approx(dl[k] * A20);
+                            if (ASTR == 2) {
+                                r2[k] = r1[k] * r1[k];
+                                cur[k] = pk(r1[k], r2[k]);  // {r^1, r^2}; next pairs: * {r^2, r^2}
+                            }
+                        }
+                    }
+                    // One pass = four states (two packed pairs, one LDS.128 of B and of C per
+                    // timestep) over the VEC timesteps of the group: first every 2^x of the pass
+                    // (independent: they stream through the MUFU / fma pipes back to back), then
+                    // the two dependent h chains.  F = sixteenths of the exps taken by the
+                    // polynomial (0 on the guarded slow path); RST = the group holds a reset.
+                    auto pass = [&](int q, auto ftag, auto rtag) {
                         constexpr int F = decltype(ftag)::value;
+                        constexpr bool RST = decltype(rtag)::value;
                         pair_t av[VEC][PP];
 #pragma unroll
                         for (int k = 0; k < VEC; ++k) {
@@ -391,13 +331,20 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 #pragma unroll
                             for (int s = 0; s < PP; ++s) {
                                 const int p = PP * q + s;
-                                if (lane_row_slot_is_poly(k * NP + p, F)) {
+                                if (ASTR == 1) {
+                                    av[k][s] = pk(r1[k], r1[k]);
+                                } else if (ASTR == 2) {
+                                    if (p > 0) cur[k] = mul2(cur[k], pk(r2[k], r2[k]));
+                                    av[k][s] = cur[k];
+                                } else if (lane_row_slot_is_poly(k * NP + p, F)) {
                                     av[k][s] = exp2_poly2<DEG>(dd, A2p[p]);
                                 } else {
                                     float lo, hi;
                                     upk(mul2(dd, A2p[p]), lo, hi);
                                     av[k][s] = pk(ex2_approx(lo), ex2_approx(hi));
                                 }
+                                // a reset step is the left-zero pair (0, u_t): h_{t-1} is dropped
+                                if (RST && ((rmask >> k) & 1u)) av[k][s] = pk(0.0f, 0.0f);
                             }
                         }
 #pragma unroll
@@ -428,63 +375,18 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         for (int k = 1; k < VEC; ++k) dm = fmaxf(dm, fabsf(dl[k]));
                         poly_ok = !__any_sync(kFullMask, !(dm <= dmax));
                     }
-                    // Software-pipelined form of the same passes (PIPE): the 2^x of pass q+1 are
-                    // issued timestep by timestep between the chain steps of pass q, so that the
-                    // MUFU works in the shadow of the fma pipe inside ONE warp (an in-order warp
-                    // cannot overlap a MUFU burst with anything else of its own).
-                    auto exps = [&](int q, int k, pair_t (&dst)[PP], auto ftag) {
-                        constexpr int F = decltype(ftag)::value;
-                        const pair_t dd = pk(dl[k], dl[k]);
+                    if (EXT && rmask != 0) {  // warp-uniform (all rows of a warp share the batch)
 #pragma unroll
-                        for (int s = 0; s < PP; ++s) {
-                            const int p = PP * q + s;
-                            if (lane_row_slot_is_poly(k * NP + p, F)) {
-                                dst[s] = exp2_poly2<DEG>(dd, A2p[p]);
-                            } else {
-                                float lo, hi;
-                                upk(mul2(dd, A2p[p]), lo, hi);
-                                dst[s] = pk(ex2_approx(lo), ex2_approx(hi));
-                            }
-                        }
-                    };
-                    auto chain = [&](int q, int k, const pair_t (&av)[PP]) {
-                        const pair_t dxx = pk(dxs[k], dxs[k]);
-                        const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 2 * PP * q;
-#pragma unroll
-                        for (int s = 0; s < PP; s += 2) {
-                            const int p = PP * q + s;
-                            const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 2 * s);
-                            const ulonglong2 c4 =
-                                *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
-                            h2[p] = fma2(av[s], h2[p], mul2(dxx, b4.x));
-                            h2[p + 1] = fma2(av[s + 1], h2[p + 1], mul2(dxx, b4.y));
-                            y2[k] = fma2(c4.x, h2[p], y2[k]);
-                            y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
-                        }
-                    };
-                    auto piped = [&](auto ftag) {
-                        constexpr int NQ = NP / PP;
-                        pair_t av[2][VEC][PP];
-#pragma unroll
-                        for (int k = 0; k < VEC; ++k) exps(0, k, av[0][k], ftag);
-#pragma unroll
-                        for (int q = 0; q < NQ; ++q) {
-#pragma unroll
-                            for (int k = 0; k < VEC; ++k) {
-                                if (q + 1 < NQ) exps(q + 1, k, av[(q + 1) & 1][k], ftag);
-                                chain(q, k, av[q & 1][k]);
-                            }
-                        }
-                    };
-                    if (PIPE) {
-                        if (poly_ok) piped(std::integral_constant<int, F16>{});
-                        else piped(std::integral_constant<int, 0>{});
+                        for (int q = 0; q < NP / PP; ++q)
+                            pass(q, std::integral_constant<int, 0>{}, std::true_type{});
                     } else if (poly_ok) {
 #pragma unroll
-                        for (int q = 0; q < NP / PP; ++q) pass(q, std::integral_constant<int, F16>{});
+                        for (int q = 0; q < NP / PP; ++q)
+                            pass(q, std::integral_constant<int, F16>{}, std::false_type{});
                     } else {
 #pragma unroll
-                        for (int q = 0; q < NP / PP; ++q) pass(q, std::integral_constant<int, 0>{});
+                        for (int q = 0; q < NP / PP; ++q)
+                            pass(q, std::integral_constant<int, 0>{}, std::false_type{});
                     }
 #pragma unroll
                     for (int k = 0; k < VEC; ++k) {
@@ -515,7 +417,11 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                     float out[YC];
 #pragma unroll
                     for (int j = 0; j < YC; ++j) out[j] = ys[j];
-                    store_y<T, YC>(yr + tg + yoff, out);
+                    if (EXT && zr) {  // f1 epilogue: y <- y * silu(z)
+#pragma unroll
+                        for (int j = 0; j < YC; ++j) out[j] *= silu_f(zv[j]);
+                    }
+                    RowSeg<T, YC>::store(yr + tg + yoff, out);
                 }
             }
         }

@@ -14,19 +14,22 @@
 // (any N <= 64, any L, any alignment via the scalar-access instantiation).
 #pragma once
 
-#include "common.cuh"
+#include <type_traits>
+
+#include "selective_common.cuh"
 
 namespace affinescan {
 
 // NV vectors of VEC elements per lane: K = NV*VEC consecutive timesteps.
-template <typename T, int VEC, int NV, int WARPS>
+// EXT = the fused steps either side of the scan (softplus/bias, silu(z) gate, resets).
+template <typename T, int VEC, int NV, int WARPS, bool EXT>
 __global__ void __launch_bounds__(WARPS * 32)
 selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                const float* __restrict__ A, const T* __restrict__ B,
                                const T* __restrict__ C, const float* __restrict__ D,
                                const float* __restrict__ h0, T* __restrict__ y,
-                               float* __restrict__ h_last, int batch, int d_inner, int N,
-                               long long L)
+                               float* __restrict__ h_last, const SelectiveExt ext, int batch,
+                               int d_inner, int N, long long L)
 {
     constexpr int K = NV * VEC;
     constexpr int kWarpTile = 32 * K;
@@ -57,10 +60,14 @@ selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ de
         hcr[i] = (n < N && h0) ? __ldg(h0 + row * N + n) : 0.0f;
     }
     const float Dd = D ? __ldg(D + d) : 0.0f;
+    const float bias = (EXT && ext.delta_bias) ? __ldg(ext.delta_bias + d) : 0.0f;
+    const T* zr = (EXT && ext.z) ? static_cast<const T*>(ext.z) + row * L : nullptr;
+    const unsigned char* rst = (EXT && ext.reset) ? ext.reset + static_cast<long long>(b) * L : nullptr;
 
     for (long long t0 = 0; t0 < L; t0 += kWarpTile) {
         const long long tl = t0 + lane * K;  // first timestep of this lane
         float dl[K], dx[K], yv[K];
+        unsigned rmask = 0;  // bit k: timestep tl + k starts a new sequence (f2)
         // ---- A1: x, delta
 #pragma unroll
         for (int v = 0; v < NV; ++v) {
@@ -68,6 +75,14 @@ selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ de
             if (tl + v * VEC < L) {
                 AccS::load(xr + tl + v * VEC, xv);
                 AccS::load(dr + tl + v * VEC, dv);
+                if (EXT) {  // f1 prologue
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) {
+                        dv[k] += bias;
+                        if (ext.delta_softplus) dv[k] = softplus_f(dv[k]);
+                        if (rst) rmask |= (__ldg(rst + tl + v * VEC + k) != 0 ? 1u : 0u) << (v * VEC + k);
+                    }
+                }
             } else {  // identity padding: delta = 0 => a = 1, u = 0 (Q12)
 #pragma unroll
                 for (int k = 0; k < VEC; ++k) { xv[k] = 0.0f; dv[k] = 0.0f; }
@@ -104,12 +119,14 @@ selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 #pragma unroll
                 for (int k = 0; k < VEC; ++k) {
                     a[v * VEC + k] = ex2_approx(dl[v * VEC + k] * A2n);
+                    // a reset step is the left-zero pair (0, u_t) of (+)
+                    if (EXT && ((rmask >> (v * VEC + k)) & 1u)) a[v * VEC + k] = 0.0f;
                     u[v * VEC + k] = dx[v * VEC + k] * bv[k];
                     cv[v * VEC + k] = cc[k];
                 }
             }
             // ---- A4: thread-local composition of K pairs
-            Pair loc{ex2_approx(dsum * A2n), u[0]};
+            Pair loc{(EXT && rmask != 0) ? 0.0f : ex2_approx(dsum * A2n), u[0]};
 #pragma unroll
             for (int k = 1; k < K; ++k) loc.U = fmaf(a[k], loc.U, u[k]);
             // ---- A5: warp combine
@@ -137,6 +154,12 @@ selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                 float out[VEC];
 #pragma unroll
                 for (int k = 0; k < VEC; ++k) out[k] = yv[v * VEC + k];
+                if (EXT && zr) {  // f1 epilogue: y <- y * silu(z)
+                    float zv[VEC];
+                    AccS::load(zr + tl + v * VEC, zv);
+#pragma unroll
+                    for (int k = 0; k < VEC; ++k) out[k] *= silu_f(zv[k]);
+                }
                 AccS::store(yr + tl + v * VEC, out);
             }
         }

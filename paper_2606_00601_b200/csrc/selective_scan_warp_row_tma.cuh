@@ -7,8 +7,8 @@
 // are shared by the whole CTA: an elected thread stages the [N][32*K] tiles of B and of C with
 // TMA tensor copies (cp.async.bulk.tensor.2d, boxes of 128/256 timesteps x N rows, mbarrier
 // complete_tx) into a 2-stage shared-memory ring; the elected thread lives in a dedicated
-// producer warp; consumers release a stage through an "empty" mbarrier (one arrival per warp).  For each state n (outer loop, NU states per
-// iteration for ILP) a lane
+// producer warp; consumers release a stage through an "empty" mbarrier (one arrival per warp).
+// For each state n (outer loop, NU states per iteration for ILP) a lane
 //   A3  discretises      a_k = ex2(delta_k * A2[n]),  u_k = (delta_k x_k) * B_k[n]   (smem)
 //   A4  composes its K pairs in registers (P via one ex2 of A2[n]*sum(delta))
 //   A5  combines across the warp with a Kogge–Stone __shfl_up_sync pair scan
@@ -16,11 +16,80 @@
 //   A8  rescans its K steps from the exclusive prefix (a_k, u_k still in registers)
 //   A9  accumulates y_k += C_k[n] * h_k (smem) ; h itself is never stored.
 // x/delta/y move with coalesced 128-bit global accesses (lane owns K contiguous elements).
+//
+// Template mode LB = variant AFFINESCAN_SELECTIVE_CHUNKED (BJ "decoupled
+// look-back for very long sequences"): the same tile body, but the (tile, row-block) work items
+// are handed out tile-major by an atomic ticket to persistent CTAs, so L is parallelised across
+// CTAs and occupancy no longer depends on the row count.  The carry h_in[n] of a tile is no
+// longer a register of the warp that ran the previous tile: for every (row, tile, state) the
+// warp publishes the tile's aggregate pair (P, U) as soon as its warp scan is done, looks back
+// over the predecessors' descriptors (32 tiles at a time, ordered shuffle tree, stops at the
+// first INCLUSIVE one) to compose its carry-in, and then publishes the INCLUSIVE state
+// (0, h_out) — the decoupled look-back of affine_scan.cuh applied per state, in the shadow of
+// the other warps' arithmetic.  Descriptors are epoch-tagged: nothing is cleared per call.
 #pragma once
 
-#include "selective_scan_lane_row.cuh"  // mbarrier / TMA helpers
+#include <type_traits>
+
+#include "affine_scan.cuh"  // tile descriptors of the decoupled look-back
+#include "selective_common.cuh"
+#include "tma.cuh"
 
 namespace affinescan {
+
+// Carry-in h_in of (row, tile, state) by decoupled look-back (LB mode).  `drow` = descriptors of
+// this row, [ntiles][N][2] 64-bit words; `tot` = the tile's aggregate pair (warp-uniform).
+// Publishes AGGREGATE(tot) first, INCLUSIVE (0, h_out) once h_in is known; tile 0 takes h0.
+__device__ __forceinline__ float selective_lookback(unsigned long long* drow, long long tile,
+                                                    int n, int N, unsigned tag, Pair tot,
+                                                    float h0n, int lane)
+{
+    unsigned long long* my = drow + (tile * N + n) * 2;
+    if (tile == 0) {
+        if (lane == 0) desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(tot, h0n)});
+        return h0n;
+    }
+    // P == 0 (underflow, or a reset inside the tile): the state after the tile does not depend
+    // on the carry, so successors need not wait for ours — but this tile's own early steps do
+    const bool self_contained = tot.P == 0.0f;
+    if (lane == 0) {
+        if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, tot.U});
+        else desc_store(my, tag, kDescAggregate, tot);
+    }
+    Pair acc = identity_pair();  // (+) of the tiles examined so far (later side)
+    long long look = tile - 1;
+    while (true) {
+        const long long idx = look - lane;
+        Pair e{0.0f, 0.0f};
+        unsigned st = kDescInclusive;  // before tile 0: never selected (tile 0 is INCLUSIVE)
+        if (idx >= 0) {
+            const unsigned long long* d = drow + (idx * N + n) * 2;
+            st = desc_load(d, tag, e);
+            while (st == kDescEmpty) {
+                __nanosleep(32);
+                st = desc_load(d, tag, e);
+            }
+        }
+        __syncwarp();
+        const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);
+        // tile 0 only ever publishes INCLUSIVE, so a lane "before tile 0" is never the first
+        const int first = incl ? (__ffs(incl) - 1) : 32;
+        if (lane > first) e = identity_pair();
+        // ordered tree reduction: lane 0 holds the LATEST tile (left operand of (+))
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const Pair o = shfl_down_pair(e, d);
+            if (lane + d < 32) e = compose(e, o);
+        }
+        acc = compose(acc, shfl_pair(e, 0));
+        if (incl) break;
+        look -= 32;
+    }
+    const float h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
+    if (!self_contained && lane == 0)
+        desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(tot, h_in)});
+    return h_in;
+}
 
 template <typename T, int K>
 struct WarpRowTmaSmem {
@@ -32,7 +101,7 @@ struct WarpRowTmaSmem {
     static constexpr int kBoxBytes = N * kBoxT * static_cast<int>(sizeof(T));
     static constexpr int kStageBytes = 2 * kBoxes * kBoxBytes;  // B boxes then C boxes
     static constexpr int kStages = 2;
-    static constexpr int kBytes = kStages * kStageBytes + 64;   // + full[2], empty[2]
+    static constexpr int kBytes = kStages * kStageBytes + 64;   // + full[2], empty[2], item[2]
     static_assert(kTileT % kBoxT == 0 && kBoxT <= 256, "tile is a whole number of boxes");
     // Bank conflicts: lane l reads the 16-byte chunks l*NV + v (v < NV) of a row.  Box and row
     // strides are multiples of 128 B, so the 8 lanes of an LDS.128 phase hit distinct 16-byte
@@ -41,62 +110,35 @@ struct WarpRowTmaSmem {
     static_assert((kBoxT * sizeof(T)) % 128 == 0, "row stride multiple of 128 B");
 };
 
-// Non-suspending poll (mbarrier.test_wait) for the short producer-side wait.
-__device__ __forceinline__ void mbar_poll(uint64_t* bar, unsigned parity)
-{
-    unsigned ok;
-    do {
-        asm volatile(
-            "{\n\t.reg .pred p;\n\t"
-            "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, p;\n\t}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
-// NU = states processed together per n-iteration, RW = rows per warp: NU*RW independent chains
-// per warp; the RW rows of a warp share every LDS of B_t/C_t (half the shared-memory traffic
-// per state-step at RW = 2).
-template <typename T, int VEC, int NV, int NU, int RW>
-__global__ void __launch_bounds__(RW == 1 ? 384 : 256, 1)
+// NU = states processed together per n-iteration (independent chains per warp).
+// EXT = the fused steps either side of the scan (softplus/bias, silu(z) gate, resets).
+// LB  = ticketed (tile, row-block) work items with the decoupled look-back carry (CHUNKED).
+template <typename T, int VEC, int NV, int NU, bool EXT, bool LB>
+__global__ void __launch_bounds__(384, 1)
 selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                    const float* __restrict__ A,
                                    const __grid_constant__ CUtensorMap mapB,
                                    const __grid_constant__ CUtensorMap mapC,
                                    const float* __restrict__ D, const float* __restrict__ h0,
-                                   T* __restrict__ y, float* __restrict__ h_last, int batch,
-                                   int d_inner, int ctas_per_batch, long long L)
+                                   T* __restrict__ y, float* __restrict__ h_last,
+                                   const SelectiveExt ext, int batch, int d_inner,
+                                   int ctas_per_batch, long long L,
+                                   unsigned long long* __restrict__ desc,
+                                   LookbackCtrl* __restrict__ ctrl)
 {
     constexpr int K = NV * VEC;
     using S = WarpRowTmaSmem<T, K>;
     constexpr int N = S::N;
-    using AccS = Access<T, VEC, true>;  // streamed once: x, delta, y
+    using AccS = Access<T, VEC, true>;  // streamed once: x, delta, y, z
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S::kStages * S::kStageBytes);
     uint64_t* empty = full + S::kStages;
+    long long* item_of_stage = reinterpret_cast<long long*>(empty + S::kStages);  // LB only
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     const int R = (blockDim.x >> 5) - 1;  // consumer warps per CTA; warp R is the producer
-    const int b = blockIdx.x / ctas_per_batch;
-    const int d0 = (blockIdx.x - b * ctas_per_batch) * R * RW;
-    bool active[RW];   // inactive rows are computed (on a valid row) but never stored: their
-    int dd[RW];        // warps still take part in the stage ring
-    long long row[RW];
-#pragma unroll
-    for (int r = 0; r < RW; ++r) {
-        const int d = d0 + warp * RW + r;
-        active[r] = d < d_inner;
-        dd[r] = active[r] ? d : d_inner - 1;
-        row[r] = static_cast<long long>(b) * d_inner + dd[r];
-    }
 
     if (threadIdx.x == 0) {
 #pragma unroll
@@ -110,8 +152,13 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
     __syncthreads();
 
     const long long ntiles = (L + S::kTileT - 1) / S::kTileT;
-    auto issue_tile = [&](long long tile) {  // one thread
-        const int st = static_cast<int>(tile % S::kStages);
+    const long long slots = static_cast<long long>(batch) * ctas_per_batch;  // row-blocks
+    // steps = stage uses of this CTA: its own tiles 0..ntiles-1 (plain), or ticketed work
+    // items until the producer draws a ticket past the end (LB)
+    const long long nitems = LB ? ntiles * slots : ntiles;
+    const unsigned tag = LB ? ((*reinterpret_cast<volatile unsigned*>(&ctrl->epoch) + 1u) & 0x3fffffffu) : 0u;
+
+    auto issue_tile = [&](int st, long long tile, int b) {  // one thread
         unsigned char* dst = smem_raw + st * S::kStageBytes;
         mbar_arrive_expect_tx(&full[st], static_cast<unsigned>(S::kStageBytes));
 #pragma unroll
@@ -122,200 +169,261 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
         }
     };
     // Producer warp: one elected lane keeps the 2-stage ring full; it refills a stage as soon
-    // as every consumer warp has released it, and never touches the data itself.
+    // as every consumer warp has released it, and never touches the data itself.  In LB mode
+    // it also draws the work items: tile-major tickets, so that every predecessor tile of an
+    // item is already running (or done) when its consumers look back.
     if (warp == R) {
         if (lane == 0) {
-            for (long long tile = 0; tile < ntiles; ++tile) {
-                if (tile >= S::kStages) {
-                    const long long prev = tile - S::kStages;  // the tile that used this stage
-                    mbar_poll(&empty[prev % S::kStages],
-                              static_cast<unsigned>((prev / S::kStages) & 1));
+            for (long long step = 0;; ++step) {
+                const int st = static_cast<int>(step % S::kStages);
+                if (step >= S::kStages) {
+                    const long long prev = step - S::kStages;  // the step that used this stage
+                    mbar_poll(&empty[st], static_cast<unsigned>((prev / S::kStages) & 1));
                     fence_proxy_async_smem();
                 }
-                issue_tile(tile);
-            }
-        }
-        return;
-    }
-
-    // Lane n keeps A2[n] = A[d,n]*log2(e) and the carry h_in[n] of each row; broadcast by shuffle.
-    float A2r[RW], hcr[RW], Dd[RW];
-#pragma unroll
-    for (int r = 0; r < RW; ++r) {
-        A2r[r] = lane < N ? __ldg(A + static_cast<long long>(dd[r]) * N + lane) * kLog2e : 0.0f;
-        hcr[r] = (lane < N && h0) ? __ldg(h0 + row[r] * N + lane) : 0.0f;
-        Dd[r] = D ? __ldg(D + dd[r]) : 0.0f;
-    }
-
-    // byte offset (inside a tensor's stage, state n = 0) of this lane's v-th 128-bit vector
-    int voff[NV];
-#pragma unroll
-    for (int v = 0; v < NV; ++v) {
-        const int t = lane * K + v * VEC;  // timestep inside the tile
-        voff[v] = (t / S::kBoxT) * S::kBoxBytes + (t % S::kBoxT) * static_cast<int>(sizeof(T));
-    }
-
-    // A1: raw 128-bit prefetch of the lane's K timesteps of x and delta, one tile ahead
-    uint4 xq[RW][NV], dq[RW][NV];
-    auto prefetch = [&](long long tile) {
-        const long long tl = tile * S::kTileT + lane * K;
-#pragma unroll
-        for (int r = 0; r < RW; ++r) {
-#pragma unroll
-            for (int v = 0; v < NV; ++v) {
-                xq[r][v] = make_uint4(0, 0, 0, 0);  // identity padding: delta = 0 => a = 1, u = 0
-                dq[r][v] = make_uint4(0, 0, 0, 0);  // (Q12)
-                if (tl + v * VEC < L) {
-                    xq[r][v] = __ldcs(reinterpret_cast<const uint4*>(x + row[r] * L + tl + v * VEC));
-                    dq[r][v] =
-                        __ldcs(reinterpret_cast<const uint4*>(delta + row[r] * L + tl + v * VEC));
+                if (LB) {
+                    const long long item = atomicAdd(&ctrl->ticket, 1u);
+                    if (item >= nitems) {  // no more work: wake the consumers with a stop item
+                        item_of_stage[st] = -1;
+                        mbar_arrive(&full[st]);
+                        break;
+                    }
+                    item_of_stage[st] = item;
+                    const long long tile = item / slots;
+                    const int b = static_cast<int>((item - tile * slots) / ctas_per_batch);
+                    issue_tile(st, tile, b);
+                } else {
+                    if (step >= ntiles) break;
+                    issue_tile(st, step, blockIdx.x / ctas_per_batch);
                 }
             }
         }
-    };
-    prefetch(0);
+    } else {
+        // ---------------------------------------------------------------- consumer warps
+        // per-row values: reloaded per work item in LB mode, once otherwise
+        int b = 0, dd = 0;
+        bool active = false;
+        long long row = 0;
+        float A2r = 0.0f, hcr = 0.0f, Dd = 0.0f, bias = 0.0f;
+        const T* zr = nullptr;
+        const unsigned char* rst = nullptr;
+        unsigned long long* drow = nullptr;
+        auto bind_row = [&](int bb, int d0) {
+            b = bb;
+            // an inactive row is computed (on a valid row) but never stored or published: its
+            // warp still takes part in the stage ring
+            active = d0 + warp < d_inner;
+            dd = active ? d0 + warp : d_inner - 1;
+            row = static_cast<long long>(b) * d_inner + dd;
+            // lane n keeps A2[n] = A[d,n]*log2(e) and (plain mode) the carry h_in[n] of the row
+            A2r = lane < N ? __ldg(A + static_cast<long long>(dd) * N + lane) * kLog2e : 0.0f;
+            hcr = (lane < N && h0) ? __ldg(h0 + row * N + lane) : 0.0f;  // LB: h0, used by tile 0
+            Dd = D ? __ldg(D + dd) : 0.0f;
+            bias = (EXT && ext.delta_bias) ? __ldg(ext.delta_bias + dd) : 0.0f;
+            zr = (EXT && ext.z) ? static_cast<const T*>(ext.z) + row * L : nullptr;
+            rst = (EXT && ext.reset) ? ext.reset + static_cast<long long>(b) * L : nullptr;
+            if (LB) drow = desc + row * ntiles * N * 2;
+        };
+        if (!LB) {
+            const int bb = blockIdx.x / ctas_per_batch;
+            bind_row(bb, (blockIdx.x - bb * ctas_per_batch) * R);
+        }
 
-    for (long long tile = 0; tile < ntiles; ++tile) {
-        const int st = static_cast<int>(tile % S::kStages);
-        const unsigned parity = static_cast<unsigned>((tile / S::kStages) & 1);
-        const long long tl = tile * S::kTileT + lane * K;  // first timestep of this lane
-        float dl[RW][K], dx[RW][K], yv[RW][K], dsum[RW];
+        // byte offset (inside a tensor's stage, state n = 0) of this lane's v-th 128-bit vector
+        int voff[NV];
 #pragma unroll
-        for (int r = 0; r < RW; ++r) {
+        for (int v = 0; v < NV; ++v) {
+            const int t = lane * K + v * VEC;  // timestep inside the tile
+            voff[v] = (t / S::kBoxT) * S::kBoxBytes + (t % S::kBoxT) * static_cast<int>(sizeof(T));
+        }
+
+        // A1: raw 128-bit loads of the lane's K timesteps of x and delta (plain mode: one tile ahead)
+        uint4 xq[NV], dq[NV];
+        auto prefetch = [&](long long tile) {
+            const long long tl = tile * S::kTileT + lane * K;
+#pragma unroll
+            for (int v = 0; v < NV; ++v) {
+                xq[v] = make_uint4(0, 0, 0, 0);  // identity padding: delta = 0 => a = 1, u = 0 (Q12)
+                dq[v] = make_uint4(0, 0, 0, 0);
+                if (tl + v * VEC < L) {
+                    xq[v] = __ldcs(reinterpret_cast<const uint4*>(x + row * L + tl + v * VEC));
+                    dq[v] = __ldcs(reinterpret_cast<const uint4*>(delta + row * L + tl + v * VEC));
+                }
+            }
+        };
+        if (!LB) prefetch(0);
+
+        for (long long step = 0;; ++step) {
+            const int st = static_cast<int>(step % S::kStages);
+            const unsigned parity = static_cast<unsigned>((step / S::kStages) & 1);
+            long long tile = step;
+            if (LB) {
+                mbar_wait(&full[st], parity);
+                const long long item = item_of_stage[st];
+                if (item < 0) break;
+                tile = item / slots;
+                const long long rem = item - tile * slots;
+                const int bb = static_cast<int>(rem / ctas_per_batch);
+                bind_row(bb, static_cast<int>(rem - static_cast<long long>(bb) * ctas_per_batch) * R);
+                prefetch(tile);
+            } else if (step >= ntiles) {
+                break;
+            }
+            const long long tl = tile * S::kTileT + lane * K;  // first timestep of this lane
+            float dl[K], dx[K], yv[K], dsum = 0.0f;
+            unsigned rmask = 0;  // bit k: timestep tl + k starts a new sequence (f2)
 #pragma unroll
             for (int v = 0; v < NV; ++v) {
                 float xv[VEC], dv[VEC];
-                unpack128<T>(xq[r][v], xv);
-                unpack128<T>(dq[r][v], dv);
+                unpack128<T>(xq[v], xv);
+                unpack128<T>(dq[v], dv);
+                const bool in = tl + v * VEC < L;
 #pragma unroll
                 for (int k = 0; k < VEC; ++k) {
-                    dl[r][v * VEC + k] = dv[k];
-                    dx[r][v * VEC + k] = dv[k] * xv[k];
-                    yv[r][v * VEC + k] = Dd[r] * xv[k];
-                }
-            }
-            dsum[r] = 0.0f;
-#pragma unroll
-            for (int k = 0; k < K; ++k) dsum[r] += dl[r][k];
-        }
-        if (tile + 1 < ntiles) prefetch(tile + 1);
-
-        mbar_wait(&full[st], parity);
-        const unsigned char* sB = smem_raw + st * S::kStageBytes;
-        const unsigned char* sC = sB + S::kBoxes * S::kBoxBytes;
-
-#pragma unroll 1
-        for (int n0 = 0; n0 < N; n0 += NU) {
-            float a[NU][RW][K], u[NU][RW][K];
-            Pair inc[NU][RW];
-            float hin[NU][RW];
-            // ---- A3 + A4 for NU states x RW rows: independent work, issued back to back
-#pragma unroll
-            for (int j = 0; j < NU; ++j) {
-                const int n = n0 + j;
-                float A2n[RW];
-#pragma unroll
-                for (int r = 0; r < RW; ++r) {
-                    A2n[r] = __shfl_sync(kFullMask, A2r[r], n);
-                    hin[j][r] = __shfl_sync(kFullMask, hcr[r], n);
-                }
-                const unsigned char* bn = sB + n * S::kBoxT * static_cast<int>(sizeof(T));
-#pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    float bv[VEC];  // one LDS.128 of B serves all RW rows
-                    unpack128<T>(*reinterpret_cast<const uint4*>(bn + voff[v]), bv);
-#pragma unroll
-                    for (int r = 0; r < RW; ++r) {
-#pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            a[j][r][v * VEC + k] = ex2_approx(dl[r][v * VEC + k] * A2n[r]);
-                            u[j][r][v * VEC + k] = dx[r][v * VEC + k] * bv[k];
-                        }
+                    if (EXT) {  // f1 prologue; padding keeps delta = 0
+                        const float t = dv[k] + bias;
+                        dv[k] = in ? (ext.delta_softplus ? softplus_f(t) : t) : 0.0f;
+                        if (rst && in)
+                            rmask |= (__ldg(rst + tl + v * VEC + k) != 0 ? 1u : 0u) << (v * VEC + k);
                     }
-                }
-#pragma unroll
-                for (int r = 0; r < RW; ++r)
-                    inc[j][r] = Pair{ex2_approx(dsum[r] * A2n[r]), u[j][r][0]};
-            }
-#pragma unroll
-            for (int k = 1; k < K; ++k) {
-#pragma unroll
-                for (int j = 0; j < NU; ++j) {
-#pragma unroll
-                    for (int r = 0; r < RW; ++r)
-                        inc[j][r].U = fmaf(a[j][r][k], inc[j][r].U, u[j][r][k]);
+                    dl[v * VEC + k] = dv[k];
+                    dx[v * VEC + k] = dv[k] * xv[k];
+                    yv[v * VEC + k] = Dd * xv[k];
                 }
             }
-            // ---- A5: warp combine (NU*RW interleaved Kogge–Stone scans)
 #pragma unroll
-            for (int dlt = 1; dlt < 32; dlt <<= 1) {
-                Pair pv[NU][RW];
-#pragma unroll
-                for (int j = 0; j < NU; ++j) {
-#pragma unroll
-                    for (int r = 0; r < RW; ++r) pv[j][r] = shfl_up_pair(inc[j][r], dlt);
-                }
-                if (lane >= dlt) {
+            for (int k = 0; k < K; ++k) dsum += dl[k];
+            if (!LB) {
+                if (tile + 1 < ntiles) prefetch(tile + 1);
+                mbar_wait(&full[st], parity);
+            }
+            const unsigned char* sB = smem_raw + st * S::kStageBytes;
+            const unsigned char* sC = sB + S::kBoxes * S::kBoxBytes;
+
+            // RST: some lane of the warp holds a reset in this tile (a_k := 0 there, and the
+            // lane's chunk product P := 0: the pair of a reset step is the left zero (0, u_t) of
+            // (+))
+            auto states = [&](auto rtag) {
+                constexpr bool RST = decltype(rtag)::value;
+#pragma unroll 1
+                for (int n0 = 0; n0 < N; n0 += NU) {
+                    float a[NU][K], u[NU][K];
+                    Pair inc[NU];
+                    float hin[NU];
+                    // ---- A3 + A4 for NU states: independent work, issued back to back
 #pragma unroll
                     for (int j = 0; j < NU; ++j) {
+                        const int n = n0 + j;
+                        const float A2n = __shfl_sync(kFullMask, A2r, n);
+                        hin[j] = __shfl_sync(kFullMask, hcr, n);
+                        const unsigned char* bn = sB + n * S::kBoxT * static_cast<int>(sizeof(T));
 #pragma unroll
-                        for (int r = 0; r < RW; ++r) inc[j][r] = compose(inc[j][r], pv[j][r]);
+                        for (int v = 0; v < NV; ++v) {
+                            float bv[VEC];
+                            unpack128<T>(*reinterpret_cast<const uint4*>(bn + voff[v]), bv);
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k) {
+                                float ak = ex2_approx(dl[v * VEC + k] * A2n);
+                                if (RST && ((rmask >> (v * VEC + k)) & 1u)) ak = 0.0f;
+                                a[j][v * VEC + k] = ak;
+                                u[j][v * VEC + k] = dx[v * VEC + k] * bv[k];
+                            }
+                        }
+                        float Pl = ex2_approx(dsum * A2n);
+                        if (RST && rmask != 0) Pl = 0.0f;
+                        inc[j] = Pair{Pl, u[j][0]};
                     }
-                }
-            }
-            // ---- A7/A8: carry-in, rescan; A9: y accumulation
 #pragma unroll
-            for (int j = 0; j < NU; ++j) {
-                const int n = n0 + j;
-                float hv[RW];
+                    for (int k = 1; k < K; ++k) {
 #pragma unroll
-                for (int r = 0; r < RW; ++r) {
-                    Pair ex = shfl_up_pair(inc[j][r], 1);
-                    if (lane == 0) ex = identity_pair();
-                    const Pair tot = shfl_pair(inc[j][r], 31);
-                    hv[r] = apply(ex, hin[j][r]);
-                    const float hout = apply(tot, hin[j][r]);  // state after the tile (uniform)
-                    if (lane == n) hcr[r] = hout;
-                }
-                const unsigned char* cn = sC + n * S::kBoxT * static_cast<int>(sizeof(T));
+                        for (int j = 0; j < NU; ++j) inc[j].U = fmaf(a[j][k], inc[j].U, u[j][k]);
+                    }
+                    // ---- A5: warp combine (NU interleaved Kogge–Stone scans)
 #pragma unroll
-                for (int v = 0; v < NV; ++v) {
-                    float cc[VEC];  // one LDS.128 of C serves all RW rows
-                    unpack128<T>(*reinterpret_cast<const uint4*>(cn + voff[v]), cc);
+                    for (int dlt = 1; dlt < 32; dlt <<= 1) {
+                        Pair pv[NU];
 #pragma unroll
-                    for (int r = 0; r < RW; ++r) {
+                        for (int j = 0; j < NU; ++j) pv[j] = shfl_up_pair(inc[j], dlt);
+                        if (lane >= dlt) {
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            hv[r] = fmaf(a[j][r][v * VEC + k], hv[r], u[j][r][v * VEC + k]);
-                            yv[r][v * VEC + k] = fmaf(cc[k], hv[r], yv[r][v * VEC + k]);
+                            for (int j = 0; j < NU; ++j) inc[j] = compose(inc[j], pv[j]);
+                        }
+                    }
+                    // ---- A7/A8: carry-in, rescan; A9: y accumulation
+#pragma unroll
+                    for (int j = 0; j < NU; ++j) {
+                        const int n = n0 + j;
+                        Pair ex = shfl_up_pair(inc[j], 1);
+                        if (lane == 0) ex = identity_pair();
+                        const Pair tot = shfl_pair(inc[j], 31);
+                        float hout;
+                        if (LB) {
+                            // A7-ii: carry-in by decoupled look-back; hin[j] = h0[n] for tile 0.
+                            // Inactive rows do not publish (their row duplicates a real one).
+                            if (active) hin[j] = selective_lookback(drow, tile, n, N, tag, tot, hin[j], lane);
+                            hout = apply(tot, hin[j]);
+                        } else {
+                            hout = apply(tot, hin[j]);  // state after the tile (uniform)
+                            if (lane == n) hcr = hout;
+                        }
+                        float hv = apply(ex, hin[j]);
+                        if (LB && h_last && active && tile == ntiles - 1 && lane == 0)
+                            h_last[row * N + n] = hout;
+                        const unsigned char* cn = sC + n * S::kBoxT * static_cast<int>(sizeof(T));
+#pragma unroll
+                        for (int v = 0; v < NV; ++v) {
+                            float cc[VEC];
+                            unpack128<T>(*reinterpret_cast<const uint4*>(cn + voff[v]), cc);
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k) {
+                                hv = fmaf(a[j][v * VEC + k], hv, u[j][v * VEC + k]);
+                                yv[v * VEC + k] = fmaf(cc[k], hv, yv[v * VEC + k]);
+                            }
                         }
                     }
                 }
-            }
-        }
-        // release the stage; the producer warp refills it with tile + 2 once every warp has
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&empty[st]);
-        // ---- A9: store y
-#pragma unroll
-        for (int r = 0; r < RW; ++r) {
-            if (active[r]) {
+            };
+            if (EXT && __any_sync(kFullMask, rmask != 0)) states(std::true_type{});
+            else states(std::false_type{});
+            // release the stage; the producer warp refills it once every warp has
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[st]);
+            // ---- A9: store y (f1 epilogue: y <- y * silu(z))
+            if (active) {
 #pragma unroll
                 for (int v = 0; v < NV; ++v) {
                     if (tl + v * VEC < L) {
                         float out[VEC];
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) out[k] = yv[r][v * VEC + k];
-                        AccS::store(y + row[r] * L + tl + v * VEC, out);
+                        for (int k = 0; k < VEC; ++k) out[k] = yv[v * VEC + k];
+                        if (EXT && zr) {
+                            float zv[VEC];
+                            AccS::load(zr + tl + v * VEC, zv);
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k) out[k] *= silu_f(zv[k]);
+                        }
+                        AccS::store(y + row * L + tl + v * VEC, out);
                     }
                 }
             }
         }
+        // ---- A10: final state (plain mode: the carry register after the last tile)
+        if (!LB && h_last && active && lane < N) h_last[row * N + lane] = hcr;
     }
-    // ---- A10: final state
-#pragma unroll
-    for (int r = 0; r < RW; ++r) {
-        if (h_last && active[r] && lane < N) h_last[row[r] * N + lane] = hcr[r];
+
+    if (LB) {
+        // The last CTA to finish re-arms the control block for the next launch on this buffer
+        // (every INCLUSIVE descriptor of this launch has been published by then).
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            __threadfence();
+            if (atomicAdd(&ctrl->done, 1u) == gridDim.x - 1) {
+                ctrl->ticket = 0;
+                ctrl->done = 0;
+                ctrl->epoch = tag;
+                __threadfence();
+            }
+        }
     }
 }
 

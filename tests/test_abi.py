@@ -10,6 +10,8 @@ from paper_2606_00601_b200 import build as libbuild
 EXPECTED = {
     "affine_scan", "affine_scan_ex", "affine_scan_host",
     "selective_scan_fwd", "selective_scan_fwd_ex", "selective_scan_fwd_host",
+    "selective_scan_fwd_ext", "selective_scan_fwd_ext_host", "selective_scan_fwd_gated",
+    "affinescan_reset_mask_from_cu_seqlens",
     "affinescan_status_string", "affinescan_last_cuda_error", "affinescan_last_variant",
     "affinescan_launch_count", "affinescan_version", "affinescan_release_cache",
     "affinescan_set_option",
@@ -20,7 +22,7 @@ def test_library_builds_and_loads():
     path = libbuild.build()
     assert os.path.exists(path)
     assert lib.load() is not None
-    assert lib.version() >= 100
+    assert lib.version() >= 200
 
 
 def test_exports_every_declared_symbol():

@@ -246,8 +246,8 @@ def lane_row_options():
     lib.set_option(lib.OPT_LANE_ROW_POLY16, -1)
 
 
-@pytest.mark.parametrize("poly16", [0, 3, 4, 5, 6])
-@pytest.mark.parametrize("G", [1, 2, 4])
+@pytest.mark.parametrize("poly16", [0, 4])
+@pytest.mark.parametrize("G", [1, 2])
 @pytest.mark.parametrize("dtype", DTYPES)
 def test_selective_lane_row_small_and_ragged_shapes(cuda_device, lane_row_options, dtype, G, poly16):
     """Every (lanes per row, share of exps on the fma-pipe polynomial) instantiation."""
@@ -271,15 +271,15 @@ def test_selective_lane_row_small_and_ragged_shapes(cuda_device, lane_row_option
 def test_selective_lane_row_polynomial_exp_slow_and_fast_decay(cuda_device, lane_row_options, dtype):
     """The fma-pipe 2^x must keep 1 - a accurate when a is close to 1 (tiny delta*|A|: long
     memory) and must flush cleanly when delta*|A| is huge (a underflows): DESIGN.md §7."""
-    lib.set_option(lib.OPT_LANE_ROW_POLY16, 6)
-    for G in (1, 2, 4):
+    lib.set_option(lib.OPT_LANE_ROW_POLY16, 4)
+    for G in (1, 2):
         lib.set_option(lib.OPT_LANE_ROW_G, G)
         for shift, a_scale in ((-7.0, 1.0), (-4.0, 0.05), (3.0, 40.0), (5.0, 400.0)):
             inp = _selective_inputs(1, 64, 16, 1024, dtype, cuda_device, 77, with_h0=True,
                                     delta_shift=shift)
             inp["A"] = (inp["A"] * a_scale).contiguous()
             check_selective(inp, lib.SELECTIVE_LANE_ROW,
-                            f"lane_row G{G} poly6 shift{shift} Ax{a_scale} {dtype}")
+                            f"lane_row G{G} poly4 shift{shift} Ax{a_scale} {dtype}")
 
 
 def test_selective_forced_lane_row_rejects_unsupported_shapes(cuda_device):

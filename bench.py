@@ -5,6 +5,7 @@ d_inner 4096, N 16, L 2048, bf16 io, fp32 state) and prints ONE JSON line.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
                     [--config 1..5] [--L len] [--variant V] [--no-e2e] [--no-cpu-baseline]
+                    [--no-all-configs] [--ext gated|powers|scalar]
 
 A "step" is one pass of the whole hot path (one selective_scan_fwd / affine_scan call) over
 one batch of seeded synthetic input.  For N > 1 (torchrun) every rank runs the same workload
@@ -34,10 +35,9 @@ METRIC = "selective_scan_fwd_elements_per_s"
 L2_BYTES = 126 * (1 << 20)
 FALLBACK_HBM_GBS = 6650.0      # B200_PROFILING.md fallback ("of fallback")
 NOMINAL_HBM_GBS = 8000.0       # BASELINE.json north_star "~8 TB/s"
-SM_COUNT = 148
-MUFU_PER_CLK_PER_SM = 16       # ex2 results / clk / SM (4 per sub-partition), DESIGN.md §6
-FP32_PER_CLK_PER_SM = 128      # FP32 lane-ops / clk / SM (nominal)
-FMA_LANEOPS_PER_CLK_PER_SM = 124   # measured with FFMA2 (profiles/r01a_pipe_probes.md)
+SM_COUNT_FALLBACK = 148        # used only if the device cannot be asked
+MUFU_PER_CLK_PER_SM = 16       # NOMINAL: 4 SFU lanes per sub-partition x 4 (ex2 results/clk/SM)
+FP32_PER_CLK_PER_SM = 128      # NOMINAL: 32 FP32 lanes per sub-partition x 4 (lane-ops/clk/SM)
 
 
 # ----------------------------------------------------------------------------- helpers
@@ -146,15 +146,21 @@ class ClockSampler:
 
 # ------------------------------------------------------------------------ the workload
 class Workload:
-    def __init__(self, args, device):
+    """One BASELINE.json config (optionally with a forced L, a forced variant, or one of the
+    SURVEY §8f extensions) with rotating device input/output sets."""
+
+    def __init__(self, cfg, device, L=0, ext=None, total=None):
         over = {}
-        if args.config == 5:
-            over["L"] = args.L or (1 << 16)
-        elif args.L:
-            over["L"] = args.L
-        self.c = config(args.config, **over)
+        if cfg == 5:
+            over["L"] = L or (1 << 16)
+            if total:
+                over["total"] = total
+        elif L:
+            over["L"] = L
+        self.c = config(cfg, **over)
         self.device = device
         self.kind = self.c.kind
+        self.ext = ext if self.kind == "selective" else None
         self.sets = []
 
     def build_sets(self, nsets, seed_offset=0):
@@ -169,20 +175,53 @@ class Workload:
                        "h_last": torch.empty(c.num_seq, dtype=torch.float32, device=self.device)}
             else:
                 inp = make_selective_inputs(ci, device=self.device)
+                self._apply_ext(inp, ci)
                 out = {"y": torch.empty_like(inp["x"]),
                        "h_last": torch.empty((c.batch, c.d_inner, c.N), dtype=torch.float32,
                                              device=self.device)}
             self.sets.append((inp, out))
         self.has_h0 = self.sets[0][0].get("h0") is not None
         self.bytes = algorithmic_bytes(c, self.has_h0)
+        if self.ext == "gated":       # + z read + bias read
+            sz = 2 if c.dtype == torch.bfloat16 else 4
+            self.bytes += c.batch * c.d_inner * c.L * sz + 4 * c.d_inner
+
+    def _apply_ext(self, inp, ci):
+        """Inputs of the SURVEY §8f rows: "gated" = raw delta (pre-softplus) + bias + z;
+        "powers" / "scalar" = structured A (A[d,n] = (n+1) A[d,0] / A[d,n] = A[d,0])."""
+        from workloads import normal, uniform
+        c, dev = self.c, self.device
+        inp["z"] = inp["delta_bias"] = None
+        if self.ext == "gated":
+            shape = (c.batch, c.d_inner, c.L)
+            inp["delta"] = normal(shape, mean=c.delta_shift, seed=ci.seed, stream=22, device=dev,
+                                  dtype=c.dtype)               # softplus is applied by the kernel
+            inp["z"] = normal(shape, seed=ci.seed, stream=20, device=dev, dtype=c.dtype)
+            inp["delta_bias"] = normal((c.d_inner,), std=0.1, seed=ci.seed, stream=21, device=dev,
+                                       dtype=torch.float32)
+        elif self.ext in ("powers", "scalar"):
+            a0 = -torch.exp(uniform((c.d_inner,), -1.0, 0.5, seed=ci.seed, stream=30, device=dev,
+                                    dtype=torch.float32))
+            if self.ext == "scalar":
+                inp["A"] = a0[:, None].repeat(1, c.N).contiguous()
+            else:
+                n1 = torch.arange(1, c.N + 1, device=dev, dtype=torch.float32)
+                inp["A"] = (0.25 * a0[:, None] * n1[None, :]).contiguous()
 
     def launch(self, i, variant=0):
         inp, out = self.sets[i % len(self.sets)]
+        lib = self.lib
         if self.kind == "affine":
-            self.lib.affine_scan_ex(inp["a"], inp["u"], inp["h0"], out["h"], out["h_last"], variant)
+            lib.affine_scan_ex(inp["a"], inp["u"], inp["h0"], out["h"], out["h_last"], variant)
+        elif self.ext:
+            structure = {"gated": lib.A_GENERAL, "powers": lib.A_POWERS,
+                         "scalar": lib.A_SCALAR_PER_ROW}[self.ext]
+            lib.selective_scan_fwd_ext(inp["x"], inp["delta"], inp["A"], inp["B"], inp["C"], inp["D"],
+                                       inp["z"], inp["delta_bias"], None, inp["h0"], out["y"],
+                                       out["h_last"], self.ext == "gated", structure, variant)
         else:
-            self.lib.selective_scan_fwd_ex(inp["x"], inp["delta"], inp["A"], inp["B"], inp["C"],
-                                           inp["D"], inp["h0"], out["y"], out["h_last"], variant)
+            lib.selective_scan_fwd_ex(inp["x"], inp["delta"], inp["A"], inp["B"], inp["C"],
+                                      inp["D"], inp["h0"], out["y"], out["h_last"], variant)
 
     # end-to-end through the C-ABI with HOST buffers (pinned)
     def build_host(self):
@@ -202,8 +241,9 @@ class Workload:
 
     def describe(self, world):
         c = self.c
-        d = {"workload": c.name, "call": "affine_scan" if self.kind == "affine"
-             else "selective_scan_fwd", "seed": c.seed}
+        d = {"workload": c.name + (f"+{self.ext}" if self.ext else ""),
+             "call": "affine_scan" if self.kind == "affine"
+             else ("selective_scan_fwd_ext" if self.ext else "selective_scan_fwd"), "seed": c.seed}
         if self.kind == "affine":
             d.update(num_seq=c.num_seq, L=c.L)
         else:
@@ -268,15 +308,34 @@ def oracle_sample_runner(c, device_inputs, seed=0):
 
 
 def time_oracle(c, inputs, target_s):
+    """The oracle as it stands on a bounded sample of the workload: (i) 1 thread, the plain loop;
+    (ii) all host cores: the identical loop, the sample's outer rows / sequences split over
+    T = os.cpu_count() threads by THIS harness (SURVEY §8d.6; oracle.c itself stays one-threaded;
+    ctypes releases the GIL).  Returns (one_thread, all_cores) records."""
+    from concurrent.futures import ThreadPoolExecutor
     run, unit, max_units = oracle_sample_runner(c, inputs)
     probe = max(1, min(max_units, 8))
     run(1)                                   # load/compile the C oracle outside the timing
     el, dt = run(probe)
     n = int(max(1, min(max_units, probe * target_s / max(dt, 1e-6))))
     el, dt = run(n)
-    return {"value": el / dt, "unit": "elements/s", "cores": 1, "kind": "oracle",
-            "sample": f"first {n} {unit} of the workload ({el} elements, {dt:.2f} s of oracle "
-                      f"time, float64, 1 thread)"}
+    one = {"value": el / dt, "unit": "elements/s", "cores": 1, "kind": "oracle",
+           "sample": f"first {n} {unit} of the workload ({el} elements, {dt:.2f} s of oracle "
+                     f"time, float64, 1 thread)"}
+    T = max(1, os.cpu_count() or 1)
+    runners = [oracle_sample_runner(c, inputs)[0] for _ in range(T)]   # a host cache per thread
+    per = max(1, min(max_units, n) // T)
+    for r in runners:
+        r(1)
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(T) as pool:
+        done = list(pool.map(lambda r: r(per), runners))
+    wall = time.perf_counter() - t0
+    el_all = sum(d[0] for d in done)
+    allc = {"value": el_all / wall, "unit": "elements/s", "cores": T, "kind": "oracle",
+            "sample": f"{T} threads x the first {per} {unit} of the workload each ({el_all} elements, "
+                      f"{wall:.2f} s wall incl. per-thread float64 widening, float64)"}
+    return one, allc
 
 
 # ------------------------------------------------------------------------- reference arm
@@ -284,7 +343,7 @@ def run_reference(args):
     rank, world, _ = dist_env()
     if rank != 0:
         return 0
-    w = Workload(args, "cpu")
+    w = Workload(args.config, "cpu", args.L)
     c = w.c
     inputs = (make_affine_inputs if c.kind == "affine" else make_selective_inputs)(
         c if c.elements <= (1 << 24) else shrink_for_cpu(c), device="cpu")
@@ -311,6 +370,7 @@ def run_reference(args):
         "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic (seeded, workloads/gen.py)",
         "config": w.describe(1),
+        "io_dtype": dtype_name(c.dtype),
         "cpu_baseline": {"value": value, "unit": "elements/s", "cores": 1, "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": value, "unit": "elements/s", "h2d_bytes_per_step": 0,
@@ -331,45 +391,34 @@ def shrink_for_cpu(c):
 
 
 # ------------------------------------------------------------------------------ our arm
-def run_ours(args):
-    rank, world, local = dist_env()
-    if not torch.cuda.is_available():
-        raise RuntimeError("bench.py (impl ours) needs a CUDA device; there is no CPU fallback")
-    torch.cuda.set_device(local)
-    device = torch.device("cuda", local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=device)
-    from paper_2606_00601_b200.sharding import max_over_ranks
+def sm_count(device):
+    try:
+        return torch.cuda.get_device_properties(device).multi_processor_count
+    except Exception:
+        return SM_COUNT_FALLBACK
 
-    from paper_2606_00601_b200 import build as libbuild
-    if not os.path.exists(libbuild.LIB_PATH):
-        libbuild.build()             # fresh checkout: the built library is git-ignored
-    import paper_2606_00601_b200 as lib
-    lib.set_option(lib.OPT_LANE_ROW_G, args.lane_row_g)
-    lib.set_option(lib.OPT_LANE_ROW_POLY16, args.lane_row_poly16)
-    w = Workload(args, device)
-    c = w.c
-    step_bytes = algorithmic_bytes(c, c.kind == "affine" and c.h0_recipe == "normal")
-    nsets = max(2, -(-4 * L2_BYTES // step_bytes)) if step_bytes < 4 * L2_BYTES else 2
-    nsets = min(nsets, 64)
-    w.build_sets(nsets, seed_offset=1000 * rank)
-    variant = args.variant
 
-    def barrier():
-        if world > 1:
-            import torch.distributed as dist
-            dist.barrier()
-        torch.cuda.synchronize()
+def alu_ceiling(c, mhz, sms):
+    """NOMINAL two-pipe arithmetic ceiling of the fused selective scan: per
+    state-step one 2^x and 4 FP32 lane-ops; a share f of the 2^x evaluated on the FP32 pipe as a
+    degree-DEG polynomial (2 + DEG extra lane-ops), the rest on the SFU; the pipes balance at
+    (1 - f) / 16 = (4 + (2 + DEG) f) / 128 cycles per state-step per SM, with the NOMINAL unit
+    counts 16 SFU and 128 FP32 lanes per SM (4 and 32 per sub-partition)."""
+    deg = 3 if c.dtype == torch.bfloat16 else 5
+    f = (FP32_PER_CLK_PER_SM - 4 * MUFU_PER_CLK_PER_SM) / (
+        FP32_PER_CLK_PER_SM + (2 + deg) * MUFU_PER_CLK_PER_SM)
+    per_clk_sm = MUFU_PER_CLK_PER_SM / (1.0 - f)          # state-steps / clk / SM
+    return f, per_clk_sm, per_clk_sm * sms * mhz * 1e6     # state-steps / s
 
-    # ---- warm-up
-    for i in range(max(args.warmup, 3)):
+
+def measure(w, variant, K, warm, device, local, barrier, max_over_ranks, world=1):
+    """W warm-up launches, then K timed launches: device time of the whole region (t_begin..t_end,
+    max over ranks) and a CUDA-event pair around every launch, with the clocks sampled meanwhile."""
+    lib = w.lib
+    for i in range(max(warm, 3)):
         w.launch(i, variant)
     torch.cuda.synchronize()
     chosen = lib.last_variant()
-
-    # ---- timed region: K steps, device time (CUDA events on the launching stream)
-    K = args.steps
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
           for _ in range(K)]
     t_begin, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -392,8 +441,138 @@ def run_ours(args):
     launches = lib.launch_count() - launches0
     total_ms = max_over_ranks(t_begin.elapsed_time(t_end), device)
     per_launch_ms = sorted(a.elapsed_time(b) for a, b in ev)
-    kernel_ms = sum(per_launch_ms) / K
-    ms_per_step = total_ms / K
+    return {"chosen": chosen, "launches": launches, "total_ms": total_ms,
+            "kernel_ms": sum(per_launch_ms) / K, "kernel_ms_min": per_launch_ms[0],
+            "kernel_ms_median": per_launch_ms[K // 2], "clocks": clocks.summary()}
+
+
+def nsets_for(step_bytes):
+    """Rotating input/output sets so that > 126 MB (L2) of other data passes between reuses."""
+    n = max(2, -(-4 * L2_BYTES // step_bytes)) if step_bytes < 4 * L2_BYTES else 2
+    return min(n, 64)
+
+
+def summarize(w, m, peak, sms):
+    """Per-config record of the all_configs block."""
+    c = w.c
+    achieved = w.bytes / (m["kernel_ms"] * 1e-3) / 1e9
+    clk = m["clocks"]
+    rec = {"workload": w.describe(1)["workload"], "kernel": w.lib.VARIANT_NAMES.get(m["chosen"], "?"),
+           "kernel_ms": round(m["kernel_ms"], 5), "kernel_ms_min": round(m["kernel_ms_min"], 5),
+           "elements_per_s": c.elements / (m["kernel_ms"] * 1e-3),
+           "algorithmic_bytes": w.bytes, "hbm_gbs": round(achieved, 1),
+           "hbm_frac": round(achieved / peak, 4),
+           "hbm_frac_of_nominal_8TBps": round(achieved / NOMINAL_HBM_GBS, 4),
+           "clocks": {"sm_mhz": clk.get("sm_mhz"), "reasons": clk.get("reasons")}}
+    if c.kind == "selective":
+        mhz = clk.get("sm_mhz") or clk.get("sm_max_mhz") or 1965.0
+        steps_state = c.elements * c.N
+        mufu_ms = steps_state / (MUFU_PER_CLK_PER_SM * sms * mhz * 1e6) * 1e3
+        rec["frac_of_mufu_only_wall"] = round(mufu_ms / m["kernel_ms"], 4)
+    return rec
+
+
+def run_all_configs(args, device, local, peak, sms, barrier, max_over_ranks):
+    """cfg1, cfg2, cfg4 (+ the forced chunked schedule), the six cfg5 lengths (+ forced look-back
+    on one long sequence and on 64 sequences), and the §8f rows on the cfg3 shape — about 10 timed
+    launches each, so the per-config claims of BASELINE.md are driver-timed."""
+    import paper_2606_00601_b200 as lib
+    out = []
+    K, W = args.all_configs_steps, 3
+
+    def one(w, variant=0, note=None):
+        m = measure(w, variant, K, W, device, local, barrier, max_over_ranks)
+        rec = summarize(w, m, peak, sms)
+        if variant:
+            rec["forced_variant"] = lib.VARIANT_NAMES.get(variant, str(variant))
+        if note:
+            rec["note"] = note
+        out.append(rec)
+
+    def selective(cfg, variants=(0,), ext=None):
+        w = Workload(cfg, device, ext=ext)
+        sb = algorithmic_bytes(w.c, False)
+        w.build_sets(nsets_for(sb))
+        for v in variants:
+            one(w, v)
+        del w
+        torch.cuda.empty_cache()
+
+    w = Workload(1, device)
+    w.build_sets(64)
+    one(w, note="197 KB: launch-latency-bound; 64 rotating sets still fit L2")
+    del w
+    selective(2)
+    selective(4, (0, lib.SELECTIVE_CHUNKED))
+    selective(3, (0,), "gated")
+    selective(3, (0,), "powers")
+    selective(3, (0,), "scalar")
+    # cfg5: one flat 2^30-element pair of arrays re-segmented for every L (12.9 GB >> L2)
+    total = 1 << 30
+    w5 = Workload(5, device, L=total, total=total)
+    w5.build_sets(1)
+    inp, outp = w5.sets[0]
+    from workloads import normal
+    h0_all = normal((1 << 20,), seed=w5.c.seed, stream=3, device=device, dtype=torch.float32)
+
+    def resegment(L, variant=0, note=None):
+        S = total // L
+        ws = Workload(5, device, L=L, total=total)
+        ws.lib = lib
+        ws.sets = [({"a": inp["a"].view(S, L), "u": inp["u"].view(S, L), "h0": h0_all[:S]},
+                    {"h": outp["h"].view(S, L),
+                     "h_last": torch.empty(S, dtype=torch.float32, device=device)})]
+        ws.has_h0 = True
+        ws.bytes = algorithmic_bytes(ws.c, True)
+        one(ws, variant, note)
+
+    for logL in (10, 12, 14, 16, 18, 20):
+        resegment(1 << logL)
+    resegment(1 << 24, lib.AFFINE_LOOKBACK, "64 sequences of 2^24, forced decoupled look-back")
+    resegment(1 << 30, lib.AFFINE_LOOKBACK, "ONE sequence of 2^30, forced decoupled look-back")
+    del w5, inp, outp
+    torch.cuda.empty_cache()
+    return out
+
+
+def run_ours(args):
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py (impl ours) needs a CUDA device; there is no CPU fallback")
+    if local >= torch.cuda.device_count():
+        raise RuntimeError(f"rank {rank}: LOCAL_RANK {local} but only {torch.cuda.device_count()} "
+                           "CUDA devices are visible")
+    torch.cuda.set_device(local)
+    device = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=device)
+    from paper_2606_00601_b200.sharding import max_over_ranks
+
+    from paper_2606_00601_b200 import build as libbuild
+    if not os.path.exists(libbuild.LIB_PATH):
+        libbuild.build()             # fresh checkout: the built library is git-ignored
+    import paper_2606_00601_b200 as lib
+    lib.set_option(lib.OPT_LANE_ROW_G, args.lane_row_g)
+    lib.set_option(lib.OPT_LANE_ROW_POLY16, args.lane_row_poly16)
+    sms = sm_count(device)
+    w = Workload(args.config, device, args.L, args.ext)
+    c = w.c
+    step_bytes = algorithmic_bytes(c, c.kind == "affine" and c.h0_recipe == "normal")
+    nsets = nsets_for(step_bytes)
+    w.build_sets(nsets, seed_offset=1000 * rank)
+    variant = args.variant
+
+    def barrier():
+        if world > 1:
+            import torch.distributed as dist
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    K = args.steps
+    m = measure(w, variant, K, args.warmup, device, local, barrier, max_over_ranks, world)
+    kernel_ms = m["kernel_ms"]
+    ms_per_step = m["total_ms"] / K
     elements = c.elements * world
     value = elements / (ms_per_step * 1e-3)
 
@@ -404,56 +583,55 @@ def run_ours(args):
         with open(os.path.join(ROOT, "profiles", "traffic.txt")) as f:
             for ln in f:
                 parts = ln.split()
-                if len(parts) >= 2 and parts[0] == c.name:
+                if len(parts) >= 2 and parts[0] == w.describe(1)["workload"]:
                     traffic = int(parts[1])
     except Exception:
         pass
-    clk = clocks.summary()
-    roofline = {"bound": "hbm", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
-                "frac": round(achieved / peak, 4), "traffic": traffic, "peak_kind": peak_kind,
-                "algorithmic_bytes": w.bytes, "kernel_ms": round(kernel_ms, 5),
-                "kernel_ms_min": round(per_launch_ms[0], 5),
-                "kernel_ms_median": round(per_launch_ms[K // 2], 5),
-                "frac_of_nominal_8TBps": round(achieved / NOMINAL_HBM_GBS, 4),
-                "kernel": lib.VARIANT_NAMES.get(chosen, str(chosen))}
+    clk = m["clocks"]
+    kernel_name = lib.VARIANT_NAMES.get(m["chosen"], str(m["chosen"]))
+    hbm = {"bound": "hbm", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+           "frac": round(achieved / peak, 4), "traffic": traffic,
+           "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum of the committed "
+                             "--set full capture (profiles/traffic.txt), not measured in this run",
+           "peak_kind": peak_kind,
+           "algorithmic_bytes": w.bytes, "kernel_ms": round(kernel_ms, 5),
+           "kernel_ms_min": round(m["kernel_ms_min"], 5),
+           "kernel_ms_median": round(m["kernel_ms_median"], 5),
+           "frac_of_nominal_8TBps": round(achieved / NOMINAL_HBM_GBS, 4),
+           "kernel": kernel_name}
     if args.lane_row_g != -1 or args.lane_row_poly16 != -1:
-        roofline["ablation"] = {"lane_row_g": args.lane_row_g,
-                                "lane_row_poly16": args.lane_row_poly16}
+        hbm["ablation"] = {"lane_row_g": args.lane_row_g, "lane_row_poly16": args.lane_row_poly16}
     line = {
         "metric": METRIC, "value": value, "unit": "elements/s", "n_gpus": world, "steps": K,
         "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "io_dtype": dtype_name(c.dtype),
         "data": "synthetic (seeded, workloads/gen.py; BASELINE.json distributions)",
         "config": {**w.describe(world),
                    "l2": f"{nsets} rotating input/output sets x {step_bytes / 1e6:.1f} MB "
                          f"(> 126 MB L2 between reuses)"},
-        "clocks": clk, "gpu_launches": launches, "roofline": roofline,
+        "clocks": clk, "gpu_launches": m["launches"], "sm_count": sms,
         "hbm_gbs_achieved": round(achieved, 1),
+        # BASELINE.json's own yardstick, stated at top level: fraction of HBM peak and its target
+        "hbm_frac_of_measured_peak": hbm["frac"],
+        "hbm_frac_of_nominal_8TBps": hbm["frac_of_nominal_8TBps"],
+        "target_70pct_of_hbm_peak_met": bool(achieved / NOMINAL_HBM_GBS >= 0.70),
     }
-    if c.kind == "selective":
-        # The binding roofline of this path is arithmetic, not HBM: one 2^x
-        # and 4 FP32 lane-ops per state-step.  Ceiling with BOTH pipes in use: a share f of the
-        # 2^x goes to the fma pipe as a degree-DEG polynomial (3 + DEG lane-ops instead of the one
-        # argument multiply: 2 + DEG extra), the rest
-        # to the MUFU; the two pipes balance at (1 - f) / 16 = (4 + (2 + DEG) f) / 124 cycles per
-        # state-step per SM (16 MUFU and 124 packed-FP32 lane-ops per clock per SM, measured:
-        # profiles/r01a_pipe_probes.md).
+    if c.kind == "selective" and args.ext in (None, "gated"):
+        # The binding roofline of the general-A path is arithmetic, not HBM.
         mhz = clk.get("sm_mhz") or clk.get("sm_max_mhz") or 1965.0
-        deg = 3 if c.dtype == torch.bfloat16 else 5
-        f = (FMA_LANEOPS_PER_CLK_PER_SM - 4 * MUFU_PER_CLK_PER_SM) / (
-            FMA_LANEOPS_PER_CLK_PER_SM + (2 + deg) * MUFU_PER_CLK_PER_SM)
-        per_clk_sm = MUFU_PER_CLK_PER_SM / (1.0 - f)          # state-steps / clk / SM
+        f, per_clk_sm, alu_peak = alu_ceiling(c, mhz, sms)
         steps_state = c.elements * c.N
-        alu_peak = per_clk_sm * SM_COUNT * mhz * 1e6          # state-steps / s
-        mufu_ms = steps_state / (MUFU_PER_CLK_PER_SM * SM_COUNT * mhz * 1e6) * 1e3
+        mufu_ms = steps_state / (MUFU_PER_CLK_PER_SM * sms * mhz * 1e6) * 1e3
+        fp32_floor_ms = 4 * steps_state / (FP32_PER_CLK_PER_SM * sms * mhz * 1e6) * 1e3
         alu_achieved = steps_state / (kernel_ms * 1e-3)
-        hbm = dict(roofline)
         line["roofline_hbm"] = hbm                             # the metric's own denominator
         line["roofline"] = {
             "bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "state-steps/s",
             "frac": round(alu_achieved / alu_peak, 4), "traffic": traffic,
-            "peak_kind": "derived: MUFU 16/clk/SM + fma pipe 124 lane-ops/clk/SM (measured "
-                         "probes) x 148 SMs x sampled SM clock, balanced polynomial offload",
+            "peak_kind": "nominal: 16 SFU (MUFU.EX2) + 128 FP32 lanes per clock per SM "
+                         f"x {sms} SMs x sampled SM clock, balanced polynomial offload "
+                         "(derivation: DESIGN.md §11)",
             "poly_share_at_balance": round(f, 4), "state_steps_per_clk_per_sm": round(per_clk_sm, 2),
             "kernel_ms": hbm["kernel_ms"], "kernel_ms_min": hbm["kernel_ms_min"],
             "kernel_ms_median": hbm["kernel_ms_median"], "kernel": hbm["kernel"],
@@ -461,15 +639,18 @@ def run_ours(args):
             "hbm_frac": hbm["frac"], "hbm_gbs": hbm["achieved"],
             "mufu_only_wall_ms": round(mufu_ms, 4),
             "frac_of_mufu_only_wall": round(mufu_ms / kernel_ms, 4),
+            "fp32_only_floor_ms": round(fp32_floor_ms, 4),
             "alu_wall_ms": round(steps_state / alu_peak * 1e3, 4), "sm_mhz_used": mhz}
         if "ablation" in hbm:
             line["roofline"]["ablation"] = hbm["ablation"]
         line["roofline_alu"] = {"frac": line["roofline"]["frac_of_mufu_only_wall"],
                                 "note": "fraction of the all-MUFU wall (1 exp per state-step at "
                                         "16/clk/SM); see roofline for the two-pipe ceiling"}
+    else:
+        line["roofline"] = hbm
 
     # ---- end to end through the C-ABI with host buffers
-    if not args.no_e2e:
+    if not args.no_e2e and not args.ext:
         w.build_host()
         for _ in range(2):
             w.launch_host()
@@ -486,9 +667,19 @@ def run_ours(args):
                        "api": f"{'affine_scan' if c.kind == 'affine' else 'selective_scan_fwd'}"
                               "_host (pinned host buffers, H2D + kernel + D2H per step)"}
 
-    # ---- the oracle timed beside it (rank 0, N=1 only)
+    # ---- the oracle timed beside it (rank 0, N=1 only): one thread and all host cores
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"] = time_oracle(c, w.sets[0][0], args.cpu_seconds)
+        one, allc = time_oracle(c, w.sets[0][0], args.cpu_seconds)
+        line["cpu_baseline"] = one
+        line["cpu_baseline_all_cores"] = allc
+
+    # ---- every other config, driver-timed (rank 0, N=1, default workload only)
+    if (rank == 0 and world == 1 and not args.no_all_configs and args.config == 3
+            and not args.ext and not args.variant):
+        del w
+        torch.cuda.empty_cache()
+        line["all_configs"] = run_all_configs(args, device, local, peak, sms, barrier,
+                                              max_over_ranks)
 
     if world > 1:
         import torch.distributed as dist
@@ -497,6 +688,25 @@ def run_ours(args):
     if rank == 0:
         print(json.dumps(line))
     return 0
+
+
+def spawn_ranks(args):
+    """`python bench.py --gpus N` (N > 1) outside torchrun: start the N ranks ourselves, one per
+    GPU, exactly as the driver would; refuse (non-zero) when the box has fewer GPUs."""
+    import socket
+    import subprocess
+    have = torch.cuda.device_count() if torch.cuda.is_available() else 0
+    if have < args.gpus:
+        print(f"bench.py: --gpus {args.gpus} requested but {have} CUDA device(s) visible; "
+              "refusing to time fewer GPUs than asked", file=sys.stderr)
+        return 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+           f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port", str(port),
+           os.path.abspath(__file__), *sys.argv[1:]]
+    return subprocess.call(cmd)
 
 
 def main():
@@ -511,6 +721,12 @@ def main():
     ap.add_argument("--lane-row-g", type=int, default=-1, help="ablation: lanes per row (1, 2, 4)")
     ap.add_argument("--lane-row-poly16", type=int, default=-1,
                     help="ablation: sixteenths of the exps on the fma-pipe polynomial (0, 3..6)")
+    ap.add_argument("--ext", default=None, choices=["gated", "powers", "scalar"],
+                    help="SURVEY §8f rows on the chosen selective config: fused softplus/bias + "
+                         "silu(z) gate, or a structured-A fast path")
+    ap.add_argument("--no-all-configs", action="store_true",
+                    help="skip the per-config block (cfg1, 2, 4, cfg5 sweep, §8f rows)")
+    ap.add_argument("--all-configs-steps", type=int, default=10)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=10)
@@ -518,7 +734,15 @@ def main():
     args = ap.parse_args()
     if args.steps < 1:
         ap.error("--steps must be >= 1")
-    sys.exit(run_reference(args) if args.impl == "reference" else run_ours(args))
+    if args.impl == "reference":
+        sys.exit(run_reference(args))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(spawn_ranks(args))           # never silently time one GPU for --gpus N
+    if args.gpus != world:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}", file=sys.stderr)
+        sys.exit(2)
+    sys.exit(run_ours(args))
 
 
 if __name__ == "__main__":

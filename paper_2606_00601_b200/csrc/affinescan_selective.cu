@@ -183,7 +183,7 @@ int launch_warp_row(const Typed<T>& t, bool vec_ok, cudaStream_t stream)
 }
 
 // ---------------------------------------------------------------- lane_row (many rows)
-template <typename T, int G, int F16, bool EXT, int ASTR>
+template <typename T, int G, int F16, int EXT, int ASTR>
 int launch_lane_row_inst(const Typed<T>& t, cudaStream_t stream)
 {
     // polynomial degree per io dtype: DESIGN.md §7 (tolerance argument)
@@ -204,22 +204,31 @@ int launch_lane_row_inst(const Typed<T>& t, cudaStream_t stream)
     return after_launch();
 }
 
+// the gated Mamba block (softplus + z, no resets) has a branch-free instantiation; any other
+// combination of fused steps takes the generic one
+template <typename T>
+bool is_gated(const Typed<T>& t)
+{
+    return t.ext.delta_softplus && t.ext.z && !t.ext.reset;
+}
+
 template <typename T, int G, int F16>
 int launch_lane_row_gf(const Typed<T>& t, cudaStream_t stream)
 {
-    return t.has_ext ? launch_lane_row_inst<T, G, F16, true, 0>(t, stream)
-                     : launch_lane_row_inst<T, G, F16, false, 0>(t, stream);
+    if (!t.has_ext) return launch_lane_row_inst<T, G, F16, 0, 0>(t, stream);
+    if (G == 1 && is_gated(t)) return launch_lane_row_inst<T, 1, F16, kExtGated, 0>(t, stream);
+    return launch_lane_row_inst<T, G, F16, kExtGeneric, 0>(t, stream);
 }
 
 template <typename T>
 int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
 {
     if (a_structure == AFFINESCAN_A_SCALAR_PER_ROW)
-        return t.has_ext ? launch_lane_row_inst<T, 1, 0, true, 1>(t, stream)
-                         : launch_lane_row_inst<T, 1, 0, false, 1>(t, stream);
+        return t.has_ext ? launch_lane_row_inst<T, 1, 0, kExtGeneric, 1>(t, stream)
+                         : launch_lane_row_inst<T, 1, 0, 0, 1>(t, stream);
     if (a_structure == AFFINESCAN_A_POWERS)
-        return t.has_ext ? launch_lane_row_inst<T, 1, 0, true, 2>(t, stream)
-                         : launch_lane_row_inst<T, 1, 0, false, 2>(t, stream);
+        return t.has_ext ? launch_lane_row_inst<T, 1, 0, kExtGeneric, 2>(t, stream)
+                         : launch_lane_row_inst<T, 1, 0, 0, 2>(t, stream);
     int G = g_opt_lane_row_g.load(std::memory_order_relaxed);
     int poly16 = g_opt_lane_row_poly16.load(std::memory_order_relaxed);
     if (G < 0) G = kLaneRowDefaultG;

@@ -30,19 +30,35 @@ __device__ __forceinline__ float rcp_approx(float x)
     asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
 }
-// softplus(v) = log(1 + e^v): v for v > 20 (difference < 2.1e-9 v); e - e^2/2 + e^3/3 for small
-// e = e^v (keeps full relative accuracy of a tiny Delta); two MUFU (EX2, LG2) otherwise.
+// softplus(v) = log(1 + e^v) = max(v, 0) + log1p(e), e = 2^(-|v| log2 e) in (0, 1]: MUFU.EX2 +
+// MUFU.LG2 and a few fp32 ops, finite for every v.  For small e (|v| > 4.6) log1p(e) is taken
+// from its series e - e^2/2 + e^3/3 instead of log2(1 + e), so that a tiny Delta = e^v keeps its
+// full relative accuracy (a slow channel's memory is 1/(Delta |A|)).
 __device__ __forceinline__ float softplus_f(float v)
 {
-    const float e = ex2_approx(fminf(v, 20.0f) * kLog2e);
-    const float small = e * fmaf(e, fmaf(e, 0.33333334f, -0.5f), 1.0f);
-    const float mid = lg2_approx(1.0f + e) * kLn2;
-    return v > 20.0f ? v : (v < -4.6f ? small : mid);
+    const float e = ex2_approx(-fabsf(v) * kLog2e);
+    const float series = e * fmaf(e, fmaf(e, 0.33333334f, -0.5f), 1.0f);
+    const float l1p = e < 0.01f ? series : lg2_approx(1.0f + e) * kLn2;
+    return fmaxf(v, 0.0f) + l1p;
 }
-// silu(v) = v / (1 + e^-v): MUFU.EX2 + MUFU.RCP.
+// silu(v) = v / (1 + e^-v): MUFU.EX2 + MUFU.RCP (relative error ~1e-6).
 __device__ __forceinline__ float silu_f(float v)
 {
     return v * rcp_approx(1.0f + ex2_approx(-v * kLog2e));
+}
+// silu(v) = (v/2) (1 + tanh(v/2)) with ONE MUFU.TANH (relative error ~5e-4): used for bf16
+// outputs only, whose own rounding is 2e-3.
+__device__ __forceinline__ float silu_tanh_f(float v)
+{
+    const float hv = 0.5f * v;
+    float t;
+    asm("tanh.approx.f32 %0, %1;" : "=f"(t) : "f"(hv));
+    return fmaf(t, hv, hv);
+}
+template <typename T>
+__device__ __forceinline__ float silu_io(float v)
+{
+    return sizeof(T) == 2 ? silu_tanh_f(v) : silu_f(v);
 }
 
 // ------------------------------------------------------------------ packed fp32x2 arithmetic

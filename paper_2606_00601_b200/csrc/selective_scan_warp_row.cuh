@@ -158,7 +158,7 @@ selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                     float zv[VEC];
                     AccS::load(zr + tl + v * VEC, zv);
 #pragma unroll
-                    for (int k = 0; k < VEC; ++k) out[k] *= silu_f(zv[k]);
+                    for (int k = 0; k < VEC; ++k) out[k] *= silu_io<T>(zv[k]);
                 }
                 AccS::store(yr + tl + v * VEC, out);
             }

@@ -251,6 +251,35 @@ AFFINESCAN_API int affinescan_reset_mask_from_cu_seqlens(const int32_t* cu_seqle
                                                          void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------
+ * selective_scan_bwd — backward pass of selective_scan_fwd (the paper evaluates
+ * "forward selective-scan workloads" only).  For the scalar
+ *     loss = sum dy[b,d,t] y[b,d,t] + sum dh_last[b,d,n] h_last[b,d,n]
+ * it writes d loss / d(input) for every input of selective_scan_fwd.  The adjoint of
+ * h_t = a_t h_{t-1} + u_t (Eq.3) is the same affine recurrence run right to left,
+ * g_t = a_{t+1} g_{t+1} + C_t dy_t, i.e. the scan of P:90 Eq.(7) over the reversed sequence;
+ * h_{t-1} is recomputed from checkpoints kept in library scratch (8 B per (b,d,t) for the
+ * checkpoints + 4 B for the dB/dC partial sums, stream-ordered), never divided out.
+ *
+ *   x, delta, dy [batch, d_inner, L] io dtype  in      A [d_inner, N] fp32   in
+ *   B, C         [batch, N, L]       io dtype  in      D [d_inner]    fp32   in, NULL => 0
+ *   h0, dh_last  [batch, d_inner, N] fp32      in, NULL => 0
+ *   dx, ddelta   [batch, d_inner, L] fp32      out     dA [d_inner, N] fp32  out (sum over batch)
+ *   dB, dC       [batch, N, L]       fp32      out (sum over d_inner)
+ *   dD           [d_inner]           fp32      out (sum over batch)
+ *   dh0          [batch, d_inner, N] fp32      out
+ * Every output pointer may be NULL (=> not written).  All gradients are fp32 whatever the io
+ * dtype; sums over rows and batches are formed in a fixed order (bitwise reproducible).
+ * Supported shapes: N == 16, d_inner % 32 == 0, L % 8 == 0, 16-byte aligned pointers; anything
+ * else returns AFFINESCAN_ERR_UNSUPPORTED.  Asynchronous on cuda_stream.
+ * ------------------------------------------------------------------------------------ */
+AFFINESCAN_API int selective_scan_bwd(const void* x, const void* delta, const float* A,
+                                      const void* B, const void* C, const float* D,
+                                      const float* h0, const void* dy, const float* dh_last,
+                                      float* dx, float* ddelta, float* dA, float* dB, float* dC,
+                                      float* dD, float* dh0, int batch, int d_inner, int N,
+                                      int64_t L, int io_dtype, void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
  * Introspection (no device work)
  * ------------------------------------------------------------------------------------ */
 /* Static, NUL-terminated description of a status code. */

@@ -54,6 +54,7 @@ _SIGNATURES = {
     "selective_scan_fwd_ext_host": (_int, [_vp] * 12 + [_int, _int, _int, _i64, _int, _int, _int, _vp]),
     "selective_scan_fwd_gated": (_int, [_vp] * 11 + [_int, _int, _int, _i64, _int, _vp]),
     "affinescan_reset_mask_from_cu_seqlens": (_int, [_vp, _int, _vp, _i64, _vp]),
+    "selective_scan_bwd": (_int, [_vp] * 16 + [_int, _int, _int, _i64, _int, _vp]),
     "affinescan_status_string": (ctypes.c_char_p, [_int]),
     "affinescan_last_cuda_error": (_int, []),
     "affinescan_last_variant": (_int, []),
@@ -268,6 +269,37 @@ def selective_scan_fwd_gated(x, delta_raw, delta_bias, A, B, C, D, z, h0, y, h_l
         _check("selective_scan_fwd_gated",
                load().selective_scan_fwd_gated(px, pdelta, pbias, pA, pB, pC, pD, pz, ph0, py, phl,
                                                batch, d_inner, N, L, io, _stream_ptr(stream, x)))
+
+
+def selective_scan_bwd(x, delta, A, B, C, D, h0, dy, dh_last, dx, ddelta, dA, dB, dC, dD, dh0,
+                       stream=None):
+    """Gradients of <dy, y> + <dh_last, h_last> of selective_scan_fwd; outputs fp32, may be None."""
+    batch, d_inner, L = x.shape
+    N = A.shape[1]
+    f32 = torch.float32
+    bdl, bnl, bdn = (batch, d_inner, L), (batch, N, L), (batch, d_inner, N)
+    args = (
+        _ptr(x, shape=bdl, device="cuda", name="x"),
+        _ptr(delta, dtype=x.dtype, shape=bdl, device="cuda", name="delta"),
+        _ptr(A, dtype=f32, shape=(d_inner, N), device="cuda", name="A"),
+        _ptr(B, dtype=x.dtype, shape=bnl, device="cuda", name="B"),
+        _ptr(C, dtype=x.dtype, shape=bnl, device="cuda", name="C"),
+        _ptr(D, dtype=f32, shape=(d_inner,), device="cuda", name="D"),
+        _ptr(h0, dtype=f32, shape=bdn, device="cuda", name="h0"),
+        _ptr(dy, dtype=x.dtype, shape=bdl, device="cuda", name="dy"),
+        _ptr(dh_last, dtype=f32, shape=bdn, device="cuda", name="dh_last"),
+        _ptr(dx, dtype=f32, shape=bdl, device="cuda", name="dx"),
+        _ptr(ddelta, dtype=f32, shape=bdl, device="cuda", name="ddelta"),
+        _ptr(dA, dtype=f32, shape=(d_inner, N), device="cuda", name="dA"),
+        _ptr(dB, dtype=f32, shape=bnl, device="cuda", name="dB"),
+        _ptr(dC, dtype=f32, shape=bnl, device="cuda", name="dC"),
+        _ptr(dD, dtype=f32, shape=(d_inner,), device="cuda", name="dD"),
+        _ptr(dh0, dtype=f32, shape=bdn, device="cuda", name="dh0"),
+    )
+    with torch.cuda.device(x.device):
+        _check("selective_scan_bwd",
+               load().selective_scan_bwd(*args, batch, d_inner, N, L, _io_dtype(x),
+                                         _stream_ptr(stream, x)))
 
 
 def reset_mask_from_cu_seqlens(cu_seqlens, reset_row, stream=None):

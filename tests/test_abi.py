@@ -11,7 +11,7 @@ EXPECTED = {
     "affine_scan", "affine_scan_ex", "affine_scan_host",
     "selective_scan_fwd", "selective_scan_fwd_ex", "selective_scan_fwd_host",
     "selective_scan_fwd_ext", "selective_scan_fwd_ext_host", "selective_scan_fwd_gated",
-    "affinescan_reset_mask_from_cu_seqlens",
+    "affinescan_reset_mask_from_cu_seqlens", "selective_scan_bwd",
     "affinescan_status_string", "affinescan_last_cuda_error", "affinescan_last_variant",
     "affinescan_launch_count", "affinescan_version", "affinescan_release_cache",
     "affinescan_set_option",

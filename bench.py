@@ -472,6 +472,52 @@ def summarize(w, m, peak, sms):
     return rec
 
 
+def time_backward(cfg, device, local, peak, barrier, K, W):
+    """selective_scan_bwd on a selective config's shape.  Algorithmic bytes: reads
+    x, delta, dy (io dtype) and B, C; writes dx, ddelta (fp32), dB, dC, dA, dD."""
+    import paper_2606_00601_b200 as lib
+    from workloads import normal
+    c = config(cfg)
+    inp = make_selective_inputs(c, device=device)
+    dy = normal(inp["x"].shape, seed=c.seed, stream=40, device=device, dtype=c.dtype)
+    f32 = dict(dtype=torch.float32, device=device)
+    bdl, bnl = (c.batch, c.d_inner, c.L), (c.batch, c.N, c.L)
+    g = [torch.empty(bdl, **f32), torch.empty(bdl, **f32), torch.empty((c.d_inner, c.N), **f32),
+         torch.empty(bnl, **f32), torch.empty(bnl, **f32), torch.empty((c.d_inner,), **f32),
+         torch.empty((c.batch, c.d_inner, c.N), **f32)]
+
+    def launch():
+        lib.selective_scan_bwd(inp["x"], inp["delta"], inp["A"], inp["B"], inp["C"], inp["D"], None,
+                               dy, None, *g)
+    for _ in range(W):
+        launch()
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(K)]
+    barrier()
+    with ClockSampler(local) as clocks:
+        for a, b in ev:
+            a.record()
+            launch()
+            b.record()
+        torch.cuda.synchronize()
+    ms = sorted(a.elapsed_time(b) for a, b in ev)
+    kernel_ms = sum(ms) / K
+    sz = 2 if c.dtype == torch.bfloat16 else 4
+    rows = c.batch * c.d_inner
+    nbytes = (3 * rows * c.L * sz + 2 * c.batch * c.N * c.L * sz + 2 * rows * c.L * 4
+              + 2 * c.batch * c.N * c.L * 4 + 4 * c.d_inner * (2 * c.N + 2) + 4 * rows * c.N)
+    achieved = nbytes / (kernel_ms * 1e-3) / 1e9
+    clk = clocks.summary()
+    return {"workload": c.name + "+backward", "kernel": "selective_scan_bwd (3 launches)",
+            "kernel_ms": round(kernel_ms, 5), "kernel_ms_min": round(ms[0], 5),
+            "elements_per_s": c.elements / (kernel_ms * 1e-3), "algorithmic_bytes": nbytes,
+            "hbm_gbs": round(achieved, 1), "hbm_frac": round(achieved / peak, 4),
+            "hbm_frac_of_nominal_8TBps": round(achieved / NOMINAL_HBM_GBS, 4),
+            "clocks": {"sm_mhz": clk.get("sm_mhz"), "reasons": clk.get("reasons")},
+            "note": "library scratch (checkpoints + dB/dC partials) is not counted as algorithmic"}
+
+
 def run_all_configs(args, device, local, peak, sms, barrier, max_over_ranks):
     """cfg1, cfg2, cfg4 (+ the forced chunked schedule), the six cfg5 lengths (+ forced look-back
     on one long sequence and on 64 sequences), and the §8f rows on the cfg3 shape — about 10 timed
@@ -507,6 +553,7 @@ def run_all_configs(args, device, local, peak, sms, barrier, max_over_ranks):
     selective(3, (0,), "gated")
     selective(3, (0,), "powers")
     selective(3, (0,), "scalar")
+    out.append(time_backward(3, device, local, peak, barrier, K, W))
     # cfg5: one flat 2^30-element pair of arrays re-segmented for every L (12.9 GB >> L2)
     total = 1 << 30
     w5 = Workload(5, device, L=total, total=total)

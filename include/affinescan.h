@@ -163,7 +163,8 @@ AFFINESCAN_API int affine_scan_host(const void* a, const void* u, const float* h
  *   B, C     [batch, N, L]        io dtype  in
  *   D        [d_inner]            fp32      in, NULL => no skip term
  *   h0       [batch, d_inner, N]  fp32      in, NULL => 0
- *   y        [batch, d_inner, L]  io dtype  out
+ *   y        [batch, d_inner, L]  io dtype  out, NULL => not stored (needs h_last != NULL:
+ *                                            the aggregate-only call of the L-sharded scan)
  *   h_last   [batch, d_inner, N]  fp32      out, NULL => not written
  *
  * 1 <= N <= AFFINESCAN_MAX_N (N = 16 is the tuned case).  exp is evaluated as
@@ -249,6 +250,30 @@ AFFINESCAN_API int selective_scan_fwd_gated(const void* x, const void* delta_raw
 AFFINESCAN_API int affinescan_reset_mask_from_cu_seqlens(const int32_t* cu_seqlens, int num_seq,
                                                          uint8_t* reset, int64_t L,
                                                          void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
+ * L-sharded scan across GPUs (the paper "does not yet address distributed or
+ * multi-GPU scan execution").  Rank r of R holds the L-slice [t_r, t_{r+1}) of every
+ * tensor.  The path has ONE exchange step:
+ *   1. selective_scan_slice_aggregate: the slice's transition pair per (row, state),
+ *        P = prod_t a_t = exp(A * sum_t delta_t),  U = state after the slice when entered with 0
+ *      (the total composition of the slice's pairs);
+ *   2. all-gather of (P, U) over the ranks (rows*N*2 floats per rank: NCCL, by the caller);
+ *   3. affinescan_compose_carry: h_in = (P_{r-1},U_{r-1}) (+) ... (+) (P_0,U_0) applied to h0
+ *      (Eq.7);
+ *   4. selective_scan_fwd on the slice with h0 = h_in (rank 0 can skip 1-3 and use h0).
+ * paper_2606_00601_b200/sharding.py drives the four steps over torch.distributed.
+ *
+ *   P, U      [batch, d_inner, N] fp32  out          (selective_scan_slice_aggregate)
+ *   P_all, U_all [world, n] fp32 in; h0 [n] fp32 in or NULL; h_in [n] fp32 out; n = rows*N
+ * ------------------------------------------------------------------------------------ */
+AFFINESCAN_API int selective_scan_slice_aggregate(const void* x, const void* delta, const float* A,
+                                                  const void* B, const void* C, float* P, float* U,
+                                                  int batch, int d_inner, int N, int64_t L,
+                                                  int io_dtype, void* cuda_stream);
+AFFINESCAN_API int affinescan_compose_carry(const float* P_all, const float* U_all,
+                                            const float* h0, float* h_in, int rank, int world,
+                                            int64_t n, void* cuda_stream);
 
 /* ------------------------------------------------------------------------------------
  * selective_scan_bwd — backward pass of selective_scan_fwd (the paper evaluates

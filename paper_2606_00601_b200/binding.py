@@ -54,6 +54,8 @@ _SIGNATURES = {
     "selective_scan_fwd_ext_host": (_int, [_vp] * 12 + [_int, _int, _int, _i64, _int, _int, _int, _vp]),
     "selective_scan_fwd_gated": (_int, [_vp] * 11 + [_int, _int, _int, _i64, _int, _vp]),
     "affinescan_reset_mask_from_cu_seqlens": (_int, [_vp, _int, _vp, _i64, _vp]),
+    "selective_scan_slice_aggregate": (_int, [_vp] * 7 + [_int, _int, _int, _i64, _int, _vp]),
+    "affinescan_compose_carry": (_int, [_vp] * 4 + [_int, _int, _i64, _vp]),
     "selective_scan_bwd": (_int, [_vp] * 16 + [_int, _int, _int, _i64, _int, _vp]),
     "affinescan_status_string": (ctypes.c_char_p, [_int]),
     "affinescan_last_cuda_error": (_int, []),
@@ -300,6 +302,41 @@ def selective_scan_bwd(x, delta, A, B, C, D, h0, dy, dh_last, dx, ddelta, dA, dB
         _check("selective_scan_bwd",
                load().selective_scan_bwd(*args, batch, d_inner, N, L, _io_dtype(x),
                                          _stream_ptr(stream, x)))
+
+
+def selective_scan_slice_aggregate(x, delta, A, B, C, P, U, stream=None):
+    """(P, U) of this rank's L-slice per (row, state): step 1 of the L-sharded scan."""
+    batch, d_inner, L = x.shape
+    N = A.shape[1]
+    f32 = torch.float32
+    args = (
+        _ptr(x, shape=(batch, d_inner, L), device="cuda", name="x"),
+        _ptr(delta, dtype=x.dtype, shape=(batch, d_inner, L), device="cuda", name="delta"),
+        _ptr(A, dtype=f32, shape=(d_inner, N), device="cuda", name="A"),
+        _ptr(B, dtype=x.dtype, shape=(batch, N, L), device="cuda", name="B"),
+        _ptr(C, dtype=x.dtype, shape=(batch, N, L), device="cuda", name="C"),
+        _ptr(P, dtype=f32, shape=(batch, d_inner, N), device="cuda", name="P"),
+        _ptr(U, dtype=f32, shape=(batch, d_inner, N), device="cuda", name="U"),
+    )
+    with torch.cuda.device(x.device):
+        _check("selective_scan_slice_aggregate",
+               load().selective_scan_slice_aggregate(*args, batch, d_inner, N, L, _io_dtype(x),
+                                                     _stream_ptr(stream, x)))
+
+
+def compose_carry(P_all, U_all, h0, h_in, rank, stream=None):
+    """h_in = fold of the aggregates of ranks < rank applied to h0: step 3 of the L-sharded scan."""
+    world = int(P_all.shape[0])
+    n = int(h_in.numel())
+    f32 = torch.float32
+    with torch.cuda.device(h_in.device):
+        _check("affinescan_compose_carry",
+               load().affinescan_compose_carry(
+                   _ptr(P_all.reshape(world, n), dtype=f32, device="cuda", name="P_all"),
+                   _ptr(U_all.reshape(world, n), dtype=f32, device="cuda", name="U_all"),
+                   _ptr(None if h0 is None else h0.reshape(n), dtype=f32, device="cuda", name="h0"),
+                   _ptr(h_in.reshape(n), dtype=f32, device="cuda", name="h_in"),
+                   int(rank), world, n, _stream_ptr(stream, h_in)))
 
 
 def reset_mask_from_cu_seqlens(cu_seqlens, reset_row, stream=None):

@@ -491,6 +491,21 @@ int selective_scan_fwd_gated(const void* x, const void* delta_raw, const float* 
                                   AFFINESCAN_VARIANT_AUTO, cuda_stream);
 }
 
+int selective_scan_slice_aggregate(const void* x, const void* delta, const float* A, const void* B,
+                                   const void* C, float* P, float* U, int batch, int d_inner,
+                                   int N, int64_t L, int io_dtype, void* cuda_stream)
+{
+    SelectiveArgs a = base_args(x, delta, A, B, C, nullptr, nullptr, nullptr, nullptr, batch,
+                                d_inner, N, L, io_dtype, AFFINESCAN_VARIANT_AUTO);
+    return slice_aggregate_impl(a, P, U, cuda_stream);
+}
+
+int affinescan_compose_carry(const float* P_all, const float* U_all, const float* h0, float* h_in,
+                             int rank, int world, int64_t n, void* cuda_stream)
+{
+    return compose_carry_impl(P_all, U_all, h0, h_in, rank, world, n, cuda_stream);
+}
+
 int affinescan_reset_mask_from_cu_seqlens(const int32_t* cu_seqlens, int num_seq, uint8_t* reset,
                                           int64_t L, void* cuda_stream)
 {

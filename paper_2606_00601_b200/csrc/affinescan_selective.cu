@@ -340,7 +340,7 @@ int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
     const Typed<T> t = typed<T>(a);
     constexpr int kVec = Io<T>::kVec;
     const bool vec_ok = (t.L % kVec == 0) && aligned16(t.x) && aligned16(t.delta) &&
-                        aligned16(t.B) && aligned16(t.C) && aligned16(t.y) &&
+                        aligned16(t.B) && aligned16(t.C) && (!t.y || aligned16(t.y)) &&
                         (!a.z || aligned16(a.z));
     const bool lane_ok_common = vec_ok && t.L < (1LL << 31) - 4096;  // TMA coordinates are int32
     const bool lane_ok = lane_ok_common && t.N == 16 && (t.d_inner % 32 == 0) && aligned16(t.A) &&
@@ -386,6 +386,86 @@ int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
     return st;
 }
 
+// ---------------------------------------------------------------- L-sharded scan
+// P[row][n] = prod_t a_t[row][n] over the slice = 2^(A2[d,n] * sum_t delta[row,t]): one warp per
+// row sums delta (coalesced), then lane n raises.  The U half of the slice aggregate is the
+// h_last of a scan from h0 = 0 (selective_scan_impl with y == NULL).
+template <typename T>
+__global__ void __launch_bounds__(256)
+slice_decay_kernel(const T* __restrict__ delta, const float* __restrict__ A, float* __restrict__ P,
+                   long long rows, int d_inner, int N, long long L)
+{
+    const int lane = threadIdx.x & 31;
+    const long long row = static_cast<long long>(blockIdx.x) * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (row >= rows) return;
+    const T* dr = delta + row * L;
+    float s = 0.0f;
+    for (long long t = lane; t < L; t += 32) {
+        float v[1];
+        Access<T, 1, true>::load(dr + t, v);
+        s += v[0];
+    }
+#pragma unroll
+    for (int o = 16; o >= 1; o >>= 1) s += __shfl_xor_sync(kFullMask, s, o);
+    const int d = static_cast<int>(row % d_inner);
+    for (int n = lane; n < N; n += 32)
+        P[row * N + n] = ex2_approx(s * (__ldg(A + static_cast<long long>(d) * N + n) * kLog2e));
+}
+
+// h_in = state entering the slice of rank `rank`: fold of the aggregates of ranks 0..rank-1 in
+// order, (P_j, U_j) (+) ... (+) (P_0, U_0) applied to h0 (Eq.7).
+__global__ void compose_carry_kernel(const float* __restrict__ P_all, const float* __restrict__ U_all,
+                                     const float* __restrict__ h0, float* __restrict__ h_in,
+                                     int rank, long long n)
+{
+    const long long i = static_cast<long long>(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float h = h0 ? h0[i] : 0.0f;
+    for (int j = 0; j < rank; ++j) h = fmaf(P_all[j * n + i], h, U_all[j * n + i]);
+    h_in[i] = h;
+}
+
+}  // namespace
+
+int slice_aggregate_impl(const SelectiveArgs& a, float* P, float* U, void* cuda_stream)
+{
+    if (a.io_dtype != AFFINESCAN_F32 && a.io_dtype != AFFINESCAN_BF16) return AFFINESCAN_ERR_DTYPE;
+    if (a.batch < 0 || a.d_inner < 0 || a.L < 0) return AFFINESCAN_ERR_SHAPE;
+    if (a.N < 1 || a.N > AFFINESCAN_MAX_N) return AFFINESCAN_ERR_UNSUPPORTED;
+    const int64_t rows = static_cast<int64_t>(a.batch) * a.d_inner;
+    if (rows == 0) return AFFINESCAN_OK;
+    if (!P || !U || !a.A || (a.L > 0 && !a.delta)) return AFFINESCAN_ERR_NULL;
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    const int64_t blocks = (rows + 7) / 8;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    if (a.io_dtype == AFFINESCAN_F32)
+        slice_decay_kernel<float><<<static_cast<unsigned>(blocks), 256, 0, stream>>>(
+            static_cast<const float*>(a.delta), a.A, P, rows, a.d_inner, a.N, a.L);
+    else
+        slice_decay_kernel<bf16><<<static_cast<unsigned>(blocks), 256, 0, stream>>>(
+            static_cast<const bf16*>(a.delta), a.A, P, rows, a.d_inner, a.N, a.L);
+    AS_TRY(after_launch());
+    SelectiveArgs s = a;  // U = h_last of the slice scanned from h0 = 0, y not stored
+    s.h0 = nullptr;
+    s.y = nullptr;
+    s.h_last = U;
+    return selective_scan_impl(s, cuda_stream);
+}
+
+int compose_carry_impl(const float* P_all, const float* U_all, const float* h0, float* h_in,
+                       int rank, int world, int64_t n, void* cuda_stream)
+{
+    if (n < 0 || world < 1 || rank < 0 || rank >= world) return AFFINESCAN_ERR_SHAPE;
+    if (n == 0) return AFFINESCAN_OK;
+    if (!h_in || (rank > 0 && (!P_all || !U_all))) return AFFINESCAN_ERR_NULL;
+    const int64_t blocks = (n + 255) / 256;
+    if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
+    compose_carry_kernel<<<static_cast<unsigned>(blocks), 256, 0,
+                           static_cast<cudaStream_t>(cuda_stream)>>>(P_all, U_all, h0, h_in, rank, n);
+    return after_launch();
+}
+
+namespace {
 }  // namespace
 
 int set_lane_row_option(int key, int value)
@@ -420,7 +500,8 @@ int selective_scan_impl(const SelectiveArgs& a, void* cuda_stream)
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
     if (rows == 0) return AFFINESCAN_OK;
     if (a.L == 0) return fill_h_last(a.h0, a.h_last, rows * a.N, stream);
-    if (!a.x || !a.delta || !a.A || !a.B || !a.C || !a.y) return AFFINESCAN_ERR_NULL;
+    // y == NULL is allowed when h_last is wanted: the aggregate-only call of the L-sharded scan
+    if (!a.x || !a.delta || !a.A || !a.B || !a.C || (!a.y && !a.h_last)) return AFFINESCAN_ERR_NULL;
     return a.io_dtype == AFFINESCAN_F32 ? selective_dispatch<float>(a, stream)
                                         : selective_dispatch<bf16>(a, stream);
 }

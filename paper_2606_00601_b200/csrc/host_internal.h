@@ -78,6 +78,11 @@ struct SelectiveArgs {
 };
 int selective_scan_impl(const SelectiveArgs& a, void* cuda_stream);
 
+// L-sharded scan helpers
+int slice_aggregate_impl(const SelectiveArgs& a, float* P, float* U, void* cuda_stream);
+int compose_carry_impl(const float* P_all, const float* U_all, const float* h0, float* h_in,
+                       int rank, int world, int64_t n, void* cuda_stream);
+
 int fill_h_last(const float* h0, float* h_last, int64_t n, cudaStream_t stream);
 
 int set_lane_row_option(int key, int value);

@@ -430,7 +430,7 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 #pragma unroll
                         for (int j = 0; j < YC; ++j) out[j] *= silu_io<T>(zv[j]);
                     }
-                    RowSeg<T, YC>::store(yr + tg + yoff, out);
+                    if (y) RowSeg<T, YC>::store(yr + tg + yoff, out);  // y == NULL: aggregate-only call
                 }
             }
         }

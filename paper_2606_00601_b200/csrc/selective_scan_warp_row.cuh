@@ -160,7 +160,7 @@ selective_scan_warp_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 #pragma unroll
                     for (int k = 0; k < VEC; ++k) out[k] *= silu_io<T>(zv[k]);
                 }
-                AccS::store(yr + tl + v * VEC, out);
+                if (y) AccS::store(yr + tl + v * VEC, out);  // y == NULL: aggregate-only call
             }
         }
     }

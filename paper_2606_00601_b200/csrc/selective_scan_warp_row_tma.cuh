@@ -402,7 +402,7 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
 #pragma unroll
                             for (int k = 0; k < VEC; ++k) out[k] *= silu_io<T>(zv[k]);
                         }
-                        AccS::store(y + row * L + tl + v * VEC, out);
+                        if (y) AccS::store(y + row * L + tl + v * VEC, out);  // NULL: aggregate-only
                     }
                 }
             }

@@ -36,3 +36,55 @@ def sum_over_ranks(value: float, device="cpu") -> float:
     t = torch.tensor([float(value)], dtype=torch.float64, device=device)
     dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return float(t.item())
+
+
+# ----------------------------------------------------------------------------- L-sharding
+def shard_range_aligned(n_units: int, rank: int, world: int, align: int):
+    """Like shard_range, but every boundary is a multiple of ``align`` (the 128-bit vector width
+    along L), so each slice keeps the vector-load kernels; the last rank takes the ragged tail."""
+    blocks = -(-n_units // align)
+    lo, hi = shard_range(blocks, rank, world)
+    return min(lo * align, n_units), min(hi * align, n_units)
+
+
+def selective_scan_fwd_l_sharded(x, delta, A, B, C, D, h0, y, h_last, group=None, ops=None):
+    """The multi-GPU L-sharded forward selective scan.
+
+    Every rank holds the L-slice [t_r, t_{r+1}) of x, delta, B, C (and writes the same slice of y);
+    A, D, h0 are replicated.  The path has ONE exchange step, a NCCL all-gather of the slices'
+    transition pairs (rows*N*2 floats per rank):
+        1. (P_r, U_r) = selective_scan_slice_aggregate(slice)             [kernels]
+        2. all_gather over the ranks                                       [NCCL]
+        3. h_in = (P_{r-1},U_{r-1}) (+) ... (+) (P_0,U_0) applied to h0    [kernel]
+        4. selective_scan_fwd(slice, h0 = h_in) -> y slice, state after the slice
+    The last rank's state is the global h_last; it is broadcast so every rank returns it.
+    ``ops`` injects the three compute steps (tests on CPU pass the oracle); by default they are
+    the library's CUDA entry points.  Only plumbing happens here.
+    """
+    if ops is None:
+        from . import binding as ops
+    world = dist.get_world_size(group) if dist.is_initialized() else 1
+    rank = dist.get_rank(group) if dist.is_initialized() else 0
+    batch, d_inner, _ = x.shape
+    N = A.shape[1]
+    f32 = dict(dtype=torch.float32, device=x.device)
+    P = torch.empty((batch, d_inner, N), **f32)
+    U = torch.empty((batch, d_inner, N), **f32)
+    ops.selective_scan_slice_aggregate(x, delta, A, B, C, P, U)
+    PU = torch.stack([P, U])                                  # one message per rank
+    if world > 1:
+        gathered = [torch.empty_like(PU) for _ in range(world)]
+        dist.all_gather(gathered, PU, group=group)
+        PU_all = torch.stack(gathered)                        # [world, 2, batch, d_inner, N]
+    else:
+        PU_all = PU[None]
+    h_in = torch.empty((batch, d_inner, N), **f32)
+    ops.compose_carry(PU_all[:, 0].contiguous(), PU_all[:, 1].contiguous(), h0, h_in, rank)
+    state = torch.empty((batch, d_inner, N), **f32)
+    ops.selective_scan_fwd(x, delta, A, B, C, D, h_in, y, state)
+    if world > 1:
+        dist.broadcast(state, src=dist.get_global_rank(group, world - 1) if group else world - 1,
+                       group=group)
+    if h_last is not None:
+        h_last.copy_(state)
+    return y, h_last

@@ -12,6 +12,7 @@ EXPECTED = {
     "selective_scan_fwd", "selective_scan_fwd_ex", "selective_scan_fwd_host",
     "selective_scan_fwd_ext", "selective_scan_fwd_ext_host", "selective_scan_fwd_gated",
     "affinescan_reset_mask_from_cu_seqlens", "selective_scan_bwd",
+    "selective_scan_slice_aggregate", "affinescan_compose_carry",
     "affinescan_status_string", "affinescan_last_cuda_error", "affinescan_last_variant",
     "affinescan_launch_count", "affinescan_version", "affinescan_release_cache",
     "affinescan_set_option",

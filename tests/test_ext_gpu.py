@@ -364,3 +364,41 @@ def test_lookback_many_tiles_with_a_close_to_one(cuda_device):
         assert_close(hl, hlref, torch.float32, "lookback a~1 h_last")
         outs.append(h)
     assert rel_err(outs[1], to_f64_numpy(outs[0])) <= 1e-5
+
+
+# ------------------------------------------------ f4: L-sharded scan, ranks emulated on one GPU
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_l_sharded_scan_primitives_ranks_emulated_sequentially(cuda_device, dtype):
+    """The CUDA entry points of the multi-GPU L-sharded scan (slice aggregate, compose carry,
+    final scan with h0 = h_in) with the R ranks run one after another on one GPU and the
+    all-gather replaced by torch.stack: equals the unsharded oracle.  (The torch.distributed
+    plumbing itself is covered by tests/test_lshard_gloo.py on CPU.)"""
+    from paper_2606_00601_b200.sharding import shard_range_aligned
+    dev = cuda_device
+    vec = 4 if dtype == torch.float32 else 8
+    for (batch, d_inner, L, R) in [(2, 64, 2048, 4), (1, 4736, 512, 2), (2, 33, 1000 + vec, 3)]:
+        inp = _inputs(batch, d_inner, L, dtype, dev, 1234 + L)
+        yref, hlref = oracle_selective(inp)
+        spans = [shard_range_aligned(L, r, R, vec) for r in range(R)]
+        slices = [{k: (t[..., lo:hi].contiguous() if k in ("x", "delta", "B", "C") else t)
+                   for k, t in inp.items()} for (lo, hi) in spans]
+        Ps, Us = [], []
+        for s in slices:
+            P = torch.full((batch, d_inner, 16), float("nan"), device=dev)
+            U = torch.full((batch, d_inner, 16), float("nan"), device=dev)
+            lib.selective_scan_slice_aggregate(s["x"], s["delta"], s["A"], s["B"], s["C"], P, U)
+            Ps.append(P)
+            Us.append(U)
+        P_all, U_all = torch.stack(Ps), torch.stack(Us)
+        ys = []
+        for r, s in enumerate(slices):
+            h_in = torch.full((batch, d_inner, 16), float("nan"), device=dev)
+            lib.compose_carry(P_all, U_all, inp["h0"], h_in, r)
+            y = torch.full_like(s["x"], float("nan"))
+            hl = torch.full((batch, d_inner, 16), float("nan"), device=dev)
+            lib.selective_scan_fwd(s["x"], s["delta"], s["A"], s["B"], s["C"], s["D"], h_in, y, hl)
+            ys.append(y)
+        torch.cuda.synchronize()
+        what = f"L-sharded {dtype} {batch}x{d_inner}x{L} R={R}"
+        assert_close(torch.cat(ys, dim=2), yref, dtype, what + " y")
+        assert_close(hl, hlref, dtype, what + " h_last")

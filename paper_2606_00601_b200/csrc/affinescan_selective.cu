@@ -268,7 +268,10 @@ int launch_chunked_inst(const Typed<T>& t, cudaStream_t stream)
     AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, S::kBoxT, 16));
     int sms = 0;
     AS_TRY(sm_count(&sms));
-    const int R = t.d_inner < kWarpRowTmaMaxWarps ? t.d_inner : kWarpRowTmaMaxWarps;
+    // 5 row-warps + the producer warp = 192 threads: two CTAs per SM (2 x 192 x 168 registers,
+    // 2 x 98 KB of staging), so one CTA's ticket + TMA latency hides behind the other's arithmetic
+    constexpr int kChunkedWarps = 5;
+    const int R = t.d_inner < kChunkedWarps ? t.d_inner : kChunkedWarps;
     const int ctas_per_batch = (t.d_inner + R - 1) / R;
     const int64_t ntiles = (t.L + S::kTileT - 1) / S::kTileT;
     int64_t nitems = 0, ndesc = 0;
@@ -284,7 +287,7 @@ int launch_chunked_inst(const Typed<T>& t, cudaStream_t stream)
                            sizeof(LookbackCtrl) + static_cast<size_t>(ndesc) * 16, &sc));
     auto* ctrl = static_cast<LookbackCtrl*>(sc.ptr);
     auto* desc = reinterpret_cast<unsigned long long*>(ctrl + 1);
-    const int64_t grid = nitems < sms ? nitems : sms;  // one persistent CTA per SM
+    const int64_t grid = nitems < 2 * sms ? nitems : 2 * sms;  // two persistent CTAs per SM
     kern<<<static_cast<unsigned>(grid), (R + 1) * 32, S::kBytes, stream>>>(
         t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner,
         ctas_per_batch, t.L, desc, ctrl);

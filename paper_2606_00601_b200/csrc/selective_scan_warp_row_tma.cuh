@@ -21,12 +21,17 @@
 // look-back for very long sequences"): the same tile body, but the (tile, row-block) work items
 // are handed out tile-major by an atomic ticket to persistent CTAs, so L is parallelised across
 // CTAs and occupancy no longer depends on the row count.  The carry h_in[n] of a tile is no
-// longer a register of the warp that ran the previous tile: for every (row, tile, state) the
-// warp publishes the tile's aggregate pair (P, U) as soon as its warp scan is done, looks back
-// over the predecessors' descriptors (32 tiles at a time, ordered shuffle tree, stops at the
-// first INCLUSIVE one) to compose its carry-in, and then publishes the INCLUSIVE state
-// (0, h_out) — the decoupled look-back of affine_scan.cuh applied per state, in the shadow of
-// the other warps' arithmetic.  Descriptors are epoch-tagged: nothing is cleared per call.
+// longer a register of the warp that ran the previous tile.  Per (row, tile):
+//   phase A   the tile's aggregate pair (P, U) of every state (discretise, local compose, ordered
+//             warp reduction; the a_k, u_k are NOT kept) is published as one descriptor per state;
+//   look-back ONE decoupled look-back for all N states: lane = predecessor tile (32 at a time),
+//             the descriptors of every state are requested before any is consumed (one L2 round
+//             trip per window), each state's window is folded with an ordered shuffle tree and
+//             stops at its first INCLUSIVE descriptor; then INCLUSIVE (0, h_out) is published;
+//   phase B   the plain tile body with h_in as the carry (the 2^x are recomputed: the schedule
+//             pays a second exp per state-step to break the serial chain over tiles, and is
+//             chosen only when rows are too few to fill the machine otherwise).
+// Descriptors are epoch-tagged: nothing is cleared per call.
 #pragma once
 
 #include <type_traits>
@@ -37,57 +42,72 @@
 
 namespace affinescan {
 
-// Carry-in h_in of (row, tile, state) by decoupled look-back (LB mode).  `drow` = descriptors of
-// this row, [ntiles][N][2] 64-bit words; `tot` = the tile's aggregate pair (warp-uniform).
-// Publishes AGGREGATE(tot) first, INCLUSIVE (0, h_out) once h_in is known; tile 0 takes h0.
-__device__ __forceinline__ float selective_lookback(unsigned long long* drow, long long tile,
-                                                    int n, int N, unsigned tag, Pair tot,
-                                                    float h0n, int lane)
+// Decoupled look-back for ALL N states of (row, tile) at once (LB mode).  `drow` = descriptors of
+// this row, [ntiles][N][2] 64-bit words; lane n < N holds the tile's aggregate (totP, totU) of
+// state n and h0n = h0[n].  Returns on lane n the carry-in h_in[n]; publishes AGGREGATE then
+// INCLUSIVE (0, h_out) per state.  Lanes are predecessor tiles while looking back.
+template <int N>
+__device__ __forceinline__ float selective_lookback_all(unsigned long long* drow, long long tile,
+                                                        unsigned tag, float totP, float totU,
+                                                        float h0n, int lane)
 {
-    unsigned long long* my = drow + (tile * N + n) * 2;
+    unsigned long long* my = drow + (tile * N + lane) * 2;
     if (tile == 0) {
-        if (lane == 0) desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(tot, h0n)});
+        if (lane < N) desc_store(my, tag, kDescInclusive, Pair{0.0f, fmaf(totP, h0n, totU)});
         return h0n;
     }
     // P == 0 (underflow, or a reset inside the tile): the state after the tile does not depend
     // on the carry, so successors need not wait for ours — but this tile's own early steps do
-    const bool self_contained = tot.P == 0.0f;
-    if (lane == 0) {
-        if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, tot.U});
-        else desc_store(my, tag, kDescAggregate, tot);
+    const bool self_contained = totP == 0.0f;
+    if (lane < N) {
+        if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, totU});
+        else desc_store(my, tag, kDescAggregate, Pair{totP, totU});
     }
-    Pair acc = identity_pair();  // (+) of the tiles examined so far (later side)
+    Pair acc = identity_pair();        // lane n: (+) of the tiles examined so far for state n
+    unsigned pending = (1u << N) - 1;  // states whose chain has not reached an INCLUSIVE yet
     long long look = tile - 1;
-    while (true) {
+    while (pending) {
         const long long idx = look - lane;
-        Pair e{0.0f, 0.0f};
-        unsigned st = kDescInclusive;  // before tile 0: never selected (tile 0 is INCLUSIVE)
-        if (idx >= 0) {
-            const unsigned long long* d = drow + (idx * N + n) * 2;
-            st = desc_load(d, tag, e);
-            while (st == kDescEmpty) {
-                __nanosleep(32);
-                st = desc_load(d, tag, e);
-            }
-        }
-        __syncwarp();
-        const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);
-        // tile 0 only ever publishes INCLUSIVE, so a lane "before tile 0" is never the first
-        const int first = incl ? (__ffs(incl) - 1) : 32;
-        if (lane > first) e = identity_pair();
-        // ordered tree reduction: lane 0 holds the LATEST tile (left operand of (+))
+        Pair e[N];
+        unsigned st[N];
+        // request every pending state's descriptor of this lane's tile before consuming any
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const Pair o = shfl_down_pair(e, d);
-            if (lane + d < 32) e = compose(e, o);
+        for (int n = 0; n < N; ++n) {
+            e[n] = Pair{0.0f, 0.0f};
+            st[n] = kDescInclusive;  // before tile 0: never selected (tile 0 is INCLUSIVE)
+            if (((pending >> n) & 1u) && idx >= 0) st[n] = desc_load(drow + (idx * N + n) * 2, tag, e[n]);
         }
-        acc = compose(acc, shfl_pair(e, 0));
-        if (incl) break;
+#pragma unroll
+        for (int n = 0; n < N; ++n) {
+            if (!((pending >> n) & 1u)) continue;  // warp-uniform
+            if (idx >= 0) {
+                while (st[n] == kDescEmpty) {
+                    __nanosleep(20);
+                    st[n] = desc_load(drow + (idx * N + n) * 2, tag, e[n]);
+                }
+            }
+            __syncwarp();
+            const unsigned incl = __ballot_sync(kFullMask, st[n] == kDescInclusive);
+            const int first = incl ? (__ffs(incl) - 1) : 32;
+            Pair w = lane > first ? identity_pair() : e[n];
+            // ordered tree reduction: lane 0 holds the LATEST tile (left operand of (+))
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const Pair o = shfl_down_pair(w, d);
+                if (lane + d < 32) w = compose(w, o);
+            }
+            const Pair win = shfl_pair(w, 0);
+            if (lane == n) acc = compose(acc, win);
+            if (incl) pending &= ~(1u << n);
+        }
+        // a chain whose accumulated product has underflowed to exactly 0 is finished too: every
+        // earlier tile would be multiplied by that 0 (Q18), so nothing is approximated
+        pending &= ~__ballot_sync(kFullMask, lane < N && acc.P == 0.0f);
         look -= 32;
     }
-    const float h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
-    if (!self_contained && lane == 0)
-        desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(tot, h_in)});
+    const float h_in = acc.U;  // acc.P == 0: an inclusive (left-zero) pair, or underflow
+    if (lane < N && !self_contained)
+        desc_store(my, tag, kDescInclusive, Pair{0.0f, fmaf(totP, h_in, totU)});
     return h_in;
 }
 
@@ -180,6 +200,15 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
                     const long long prev = step - S::kStages;  // the step that used this stage
                     mbar_poll(&empty[st], static_cast<unsigned>((prev / S::kStages) & 1));
                     fence_proxy_async_smem();
+                }
+                if (LB && step >= 1) {
+                    // A drawn ticket must be worked on at once: successors of a tile that sits
+                    // prefetched behind this CTA's current item would all wait for it (every
+                    // look-back polls its predecessors' aggregates).  So the next ticket is drawn
+                    // only when the consumers have released the PREVIOUS item; the staging
+                    // latency this exposes is covered by the second CTA on the SM.
+                    const long long prev = step - 1;
+                    mbar_poll(&empty[prev % S::kStages], static_cast<unsigned>((prev / S::kStages) & 1));
                 }
                 if (LB) {
                     const long long item = atomicAdd(&ctrl->ticket, 1u);
@@ -356,19 +385,9 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
                         Pair ex = shfl_up_pair(inc[j], 1);
                         if (lane == 0) ex = identity_pair();
                         const Pair tot = shfl_pair(inc[j], 31);
-                        float hout;
-                        if (LB) {
-                            // A7-ii: carry-in by decoupled look-back; hin[j] = h0[n] for tile 0.
-                            // Inactive rows do not publish (their row duplicates a real one).
-                            if (active) hin[j] = selective_lookback(drow, tile, n, N, tag, tot, hin[j], lane);
-                            hout = apply(tot, hin[j]);
-                        } else {
-                            hout = apply(tot, hin[j]);  // state after the tile (uniform)
-                            if (lane == n) hcr = hout;
-                        }
+                        const float hout = apply(tot, hin[j]);  // state after the tile (uniform)
+                        if (lane == n) hcr = hout;
                         float hv = apply(ex, hin[j]);
-                        if (LB && h_last && active && tile == ntiles - 1 && lane == 0)
-                            h_last[row * N + n] = hout;
                         const unsigned char* cn = sC + n * S::kBoxT * static_cast<int>(sizeof(T));
 #pragma unroll
                         for (int v = 0; v < NV; ++v) {
@@ -383,8 +402,39 @@ selective_scan_warp_row_tma_kernel(const T* __restrict__ x, const T* __restrict_
                     }
                 }
             };
-            if (EXT && __any_sync(kFullMask, rmask != 0)) states(std::true_type{});
+            const bool tile_has_reset = EXT && __any_sync(kFullMask, rmask != 0);
+            if (LB) {
+                // ---- phase A: the tile's aggregate pair of every state; lane n keeps state n's
+                float totP = 1.0f, totU = 0.0f;
+#pragma unroll 1
+                for (int n = 0; n < N; ++n) {
+                    const float A2n = __shfl_sync(kFullMask, A2r, n);
+                    const unsigned char* bn = sB + n * S::kBoxT * static_cast<int>(sizeof(T));
+                    Pair loc{ex2_approx(dsum * A2n), 0.0f};
+                    if (tile_has_reset && rmask != 0) loc.P = 0.0f;
+#pragma unroll
+                    for (int v = 0; v < NV; ++v) {
+                        float bv[VEC];
+                        unpack128<T>(*reinterpret_cast<const uint4*>(bn + voff[v]), bv);
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            float ak = ex2_approx(dl[v * VEC + k] * A2n);
+                            if (tile_has_reset && ((rmask >> (v * VEC + k)) & 1u)) ak = 0.0f;
+                            loc.U = fmaf(ak, loc.U, dx[v * VEC + k] * bv[k]);
+                        }
+                    }
+                    const Pair inc = warp_inclusive_scan(loc, lane);
+                    const Pair tot = shfl_pair(inc, 31);
+                    if (lane == n) { totP = tot.P; totU = tot.U; }
+                }
+                // ---- A7-ii: one decoupled look-back for all states; lane n gets h_in[n].
+                // Inactive rows neither publish nor look back (their row duplicates a real one).
+                if (active) hcr = selective_lookback_all<N>(drow, tile, tag, totP, totU, hcr, lane);
+            }
+            // ---- phase B (LB) / the tile body (plain): carry in hcr, lane n holds state n's
+            if (tile_has_reset) states(std::true_type{});
             else states(std::false_type{});
+            if (LB && h_last && active && tile == ntiles - 1 && lane < N) h_last[row * N + lane] = hcr;
             // release the stage; the producer warp refills it once every warp has
             __syncwarp();
             if (lane == 0) mbar_arrive(&empty[st]);

@@ -672,27 +672,25 @@ def run_ours(args):
         mufu_ms = steps_state / (MUFU_PER_CLK_PER_SM * sms * mhz * 1e6) * 1e3
         fp32_floor_ms = 4 * steps_state / (FP32_PER_CLK_PER_SM * sms * mhz * 1e6) * 1e3
         alu_achieved = steps_state / (kernel_ms * 1e-3)
-        line["roofline_hbm"] = hbm                             # the metric's own denominator
-        line["roofline"] = {
+        # BASELINE.json's metric is the HBM fraction, so `roofline` stays the HBM view;
+        # the arithmetic ceiling that actually binds this path is reported beside it.
+        line["roofline"] = hbm
+        line["roofline_alu"] = {
             "bound": "alu", "achieved": alu_achieved, "peak": alu_peak, "unit": "state-steps/s",
-            "frac": round(alu_achieved / alu_peak, 4), "traffic": traffic,
+            "frac": round(alu_achieved / alu_peak, 4),
             "peak_kind": "nominal: 16 SFU (MUFU.EX2) + 128 FP32 lanes per clock per SM "
                          f"x {sms} SMs x sampled SM clock, balanced polynomial offload "
                          "(derivation: DESIGN.md §11)",
             "poly_share_at_balance": round(f, 4), "state_steps_per_clk_per_sm": round(per_clk_sm, 2),
-            "kernel_ms": hbm["kernel_ms"], "kernel_ms_min": hbm["kernel_ms_min"],
-            "kernel_ms_median": hbm["kernel_ms_median"], "kernel": hbm["kernel"],
-            "algorithmic_bytes": w.bytes,
-            "hbm_frac": hbm["frac"], "hbm_gbs": hbm["achieved"],
+            "kernel_ms": hbm["kernel_ms"], "kernel": hbm["kernel"],
             "mufu_only_wall_ms": round(mufu_ms, 4),
             "frac_of_mufu_only_wall": round(mufu_ms / kernel_ms, 4),
             "fp32_only_floor_ms": round(fp32_floor_ms, 4),
-            "alu_wall_ms": round(steps_state / alu_peak * 1e3, 4), "sm_mhz_used": mhz}
+            "alu_wall_ms": round(steps_state / alu_peak * 1e3, 4), "sm_mhz_used": mhz,
+            "note": "the general-A selective scan needs N exp and 4N FP32 lane-ops per element: "
+                    "its arithmetic floor lies above the HBM floor (DESIGN.md §6.2)"}
         if "ablation" in hbm:
-            line["roofline"]["ablation"] = hbm["ablation"]
-        line["roofline_alu"] = {"frac": line["roofline"]["frac_of_mufu_only_wall"],
-                                "note": "fraction of the all-MUFU wall (1 exp per state-step at "
-                                        "16/clk/SM); see roofline for the two-pipe ceiling"}
+            line["roofline_alu"]["ablation"] = hbm["ablation"]
     else:
         line["roofline"] = hbm
 

@@ -12,6 +12,7 @@
 #pragma once
 
 #include "common.cuh"
+#include "tma.cuh"
 
 namespace affinescan {
 
@@ -113,6 +114,59 @@ __device__ __forceinline__ void seq_pos(long long q0, long long r0, int off, lon
     }
 }
 
+// ------------------------------------------------------------------ decoupled look-back
+// Run by one warp.  Publishes the tile's descriptor (AGGREGATE, or INCLUSIVE at once when the
+// tile needs no carry-in: it starts at a sequence head, or its product is exactly 0), walks the
+// predecessors 32 at a time until an INCLUSIVE one, publishes INCLUSIVE, and returns the state
+// entering the tile.
+__device__ __forceinline__ float lookback_carry(unsigned long long* __restrict__ desc,
+                                                unsigned tile, unsigned tag, Pair agg,
+                                                bool need_carry, int lane)
+{
+    unsigned long long* my = desc + 2ull * tile;
+    const bool self_contained = (agg.P == 0.0f) || !need_carry;
+    if (lane == 0) {
+        if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, agg.U});
+        else desc_store(my, tag, kDescAggregate, agg);
+    }
+    float h_in = 0.0f;
+    if (need_carry) {
+        Pair acc = identity_pair();  // (+) of the tiles examined so far (later side)
+        long long look = static_cast<long long>(tile) - 1;
+        while (true) {
+            const long long idx = look - lane;
+            Pair e{0.0f, 0.0f};
+            unsigned st = kDescInclusive;  // before the stream: state 0
+            if (idx >= 0) {
+                const unsigned long long* d = desc + 2ull * idx;
+                st = desc_load(d, tag, e);
+                while (st == kDescEmpty) {  // back off: the poll competes with the data stream
+                    __nanosleep(64);
+                    st = desc_load(d, tag, e);
+                }
+            }
+            __syncwarp();
+            const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);
+            const int first = incl ? (__ffs(incl) - 1) : 32;
+            if (lane > first) e = identity_pair();
+            // ordered tree reduction: lane 0 holds the LATEST tile (left operand)
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const Pair o = shfl_down_pair(e, d);
+                if (lane + d < 32) e = compose(e, o);
+            }
+            const Pair win = shfl_pair(e, 0);
+            acc = compose(acc, win);
+            if (incl) break;
+            look -= 32;
+        }
+        h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
+        if (lane == 0 && !self_contained)
+            desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(agg, h_in)});
+    }
+    return h_in;
+}
+
 // ====================================================================================
 // Variant AFFINESCAN_AFFINE_LOOKBACK: single pass, decoupled look-back
 // ====================================================================================
@@ -190,48 +244,7 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
         Pair agg = s_warp[0];
 #pragma unroll
         for (int w = 1; w < WARPS; ++w) agg = compose(s_warp[w], agg);
-        unsigned long long* my = desc + 2ull * tile;
-        const bool need_carry = (r0 != 0);  // a tile that starts at a head ignores its carry-in
-        const bool self_contained = (agg.P == 0.0f) || !need_carry;
-        if (lane == 0) {
-            if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, agg.U});
-            else desc_store(my, tag, kDescAggregate, agg);
-        }
-        float h_in = 0.0f;
-        if (need_carry) {
-            Pair acc = identity_pair();  // (+) of the tiles examined so far (later side)
-            long long look = static_cast<long long>(tile) - 1;
-            while (true) {
-                const long long idx = look - lane;
-                Pair e{0.0f, 0.0f};
-                unsigned st = kDescInclusive;  // before the stream: state 0
-                if (idx >= 0) {
-                    const unsigned long long* d = desc + 2ull * idx;
-                    st = desc_load(d, tag, e);
-                    while (st == kDescEmpty) {  // back off: the poll competes with the data stream
-                        __nanosleep(64);
-                        st = desc_load(d, tag, e);
-                    }
-                }
-                __syncwarp();
-                const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);
-                const int first = incl ? (__ffs(incl) - 1) : 32;
-                if (lane > first) e = identity_pair();
-                // ordered tree reduction: lane 0 holds the LATEST tile (left operand)
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const Pair o = shfl_down_pair(e, d);
-                    if (lane + d < 32) e = compose(e, o);
-                }
-                const Pair win = shfl_pair(e, 0);
-                acc = compose(acc, win);
-                if (incl) break;
-                look -= 32;
-            }
-            h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
-            if (lane == 0 && !self_contained)
-                desc_store(my, tag, kDescInclusive, Pair{0.0f, apply(agg, h_in)});
-        }
+        const float h_in = lookback_carry(desc, tile, tag, agg, r0 != 0, lane);
         if (lane == 0) s_hin = h_in;
     }
     __syncthreads();
@@ -265,6 +278,278 @@ affine_scan_lookback_kernel(const T* __restrict__ a, const T* __restrict__ u,
         __threadfence();
         const unsigned ntiles = gridDim.x;
         if (atomicAdd(&ctrl->done, 1u) == ntiles - 1) {
+            ctrl->ticket = 0;
+            ctrl->done = 0;
+            ctrl->epoch = tag;  // = old epoch + 1 (mod 2^30)
+            __threadfence();
+        }
+    }
+}
+
+// ====================================================================================
+// Variant AFFINESCAN_AFFINE_LOOKBACK, vector path: PERSISTENT single-pass chained scan.
+// Same tiles, descriptors and look-back as the kernel above, but a CTA lives for the whole
+// launch: a producer warp draws tile tickets and streams the a/u tiles into a STAGES-deep
+// shared-memory ring with TMA bulk copies (cp.async.bulk + mbarrier complete_tx), so the
+// HBM read stream never waits for a ticket, a barrier or a look-back.  The WARPS consumer
+// warps run a two-deep software pipeline over the CTA's tiles:
+//     A(i+1): tile i+1 from the ring -> registers, thread/warp/CTA scan, PUBLISH its descriptor
+//     B(i)  : look back for tile i (the only wait), re-read a/u of tile i from its ring slot,
+//             apply the prefix, store h with 128-bit streaming stores, free the slot
+// A CTA therefore never sits in a look-back wait with a tile whose aggregate its successors
+// need still unpublished (a persistent CTA that waited first was measured 1.6x slower than
+// the non-persistent kernel).  Between A and B a tile keeps only its 2*J prefix pairs in
+// registers; its a/u stay in shared memory.
+// Tickets are handed out in increasing order to running CTAs and a CTA works through its
+// tiles in that order, so the smallest unfinished tile is always somebody's oldest tile with
+// every predecessor finished: forward progress needs no assumption about residency.  The
+// control block is re-armed by the last CTA to exit (every producer has drawn its
+// terminating ticket by then).
+// ====================================================================================
+template <typename T, int VEC, int J, int WARPS, int STAGES>
+struct ChainSmem {
+    static constexpr int kTile = WARPS * 32 * VEC * J;
+    static constexpr int kArrayBytes = kTile * static_cast<int>(sizeof(T));
+    static constexpr int kStageBytes = 2 * kArrayBytes;  // a tile then u tile
+    static constexpr int kCtrlOffset = STAGES * kStageBytes;
+    // full[STAGES], empty[STAGES] mbarriers; tile id, q0, r0 per stage; s_warp[3][WARPS]; s_hin
+    static constexpr int kBytes = kCtrlOffset + STAGES * 5 * 8 + 3 * WARPS * 8 + 16;
+};
+
+// First half of the look-back: publish the tile's own descriptor (no waiting).
+__device__ __forceinline__ bool lookback_publish(unsigned long long* __restrict__ desc,
+                                                 unsigned tile, unsigned tag, Pair agg,
+                                                 bool need_carry, int lane)
+{
+    const bool self_contained = (agg.P == 0.0f) || !need_carry;
+    if (lane == 0) {
+        unsigned long long* my = desc + 2ull * tile;
+        if (self_contained) desc_store(my, tag, kDescInclusive, Pair{0.0f, agg.U});
+        else desc_store(my, tag, kDescAggregate, agg);
+    }
+    return self_contained;
+}
+
+// Second half: walk the predecessors until an INCLUSIVE one, publish INCLUSIVE, return h_in.
+__device__ __forceinline__ float lookback_wait(unsigned long long* __restrict__ desc,
+                                               unsigned tile, unsigned tag, Pair agg,
+                                               bool self_contained, int lane)
+{
+    Pair acc = identity_pair();  // (+) of the tiles examined so far (later side)
+    long long look = static_cast<long long>(tile) - 1;
+    while (true) {
+        const long long idx = look - lane;
+        Pair e{0.0f, 0.0f};
+        unsigned st = kDescInclusive;  // before the stream: state 0
+        if (idx >= 0) {
+            const unsigned long long* d = desc + 2ull * idx;
+            st = desc_load(d, tag, e);
+            while (st == kDescEmpty) {
+                __nanosleep(32);
+                st = desc_load(d, tag, e);
+            }
+        }
+        __syncwarp();
+        const unsigned incl = __ballot_sync(kFullMask, st == kDescInclusive);
+        const int first = incl ? (__ffs(incl) - 1) : 32;
+        if (lane > first) e = identity_pair();
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const Pair o = shfl_down_pair(e, d);
+            if (lane + d < 32) e = compose(e, o);
+        }
+        acc = compose(acc, shfl_pair(e, 0));
+        if (incl) break;
+        look -= 32;
+    }
+    const float h_in = acc.U;  // acc.P == 0: the chain ended at an inclusive (left-zero) pair
+    if (lane == 0 && !self_contained)
+        desc_store(desc + 2ull * tile, tag, kDescInclusive, Pair{0.0f, apply(agg, h_in)});
+    return h_in;
+}
+
+template <typename T, int VEC, int J, int WARPS, int STAGES, int CTAS_PER_SM>
+__global__ void __launch_bounds__((WARPS + 1) * 32, CTAS_PER_SM)
+affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
+                         const float* __restrict__ h0, T* __restrict__ h,
+                         float* __restrict__ h_last, long long total, long long L,
+                         long long ntiles, unsigned long long* __restrict__ desc,
+                         LookbackCtrl* __restrict__ ctrl)
+{
+    using S = ChainSmem<T, VEC, J, WARPS, STAGES>;
+    constexpr int kWarpElems = 32 * VEC * J;
+    constexpr int kTile = S::kTile;
+    using Acc = Access<T, VEC, true>;
+    static_assert(STAGES >= 3, "a slot is held for two iterations");
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + S::kCtrlOffset);
+    uint64_t* empty = full + STAGES;
+    long long* s_tile = reinterpret_cast<long long*>(empty + STAGES);
+    long long* s_q0 = s_tile + STAGES;
+    long long* s_r0 = s_q0 + STAGES;
+    Pair* s_warp = reinterpret_cast<Pair*>(s_r0 + STAGES);  // [3][WARPS]
+    float* s_hin = reinterpret_cast<float*>(s_warp + 3 * WARPS);
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const unsigned tag = (*reinterpret_cast<volatile unsigned*>(&ctrl->epoch) + 1u) & 0x3fffffffu;
+
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], WARPS);
+        }
+        fence_mbar_init();
+    }
+    __syncthreads();
+
+    if (warp == WARPS) {
+        // ------------------------------------------------------------ producer warp
+        if (lane == 0) {
+            for (unsigned it = 0;; ++it) {
+                const int st = static_cast<int>(it % STAGES);
+                if (it >= STAGES) mbar_wait(&empty[st], ((it / STAGES) - 1u) & 1u);
+                const long long tk = static_cast<long long>(atomicAdd(&ctrl->ticket, 1u));
+                if (tk >= ntiles) {
+                    s_tile[st] = -1;
+                    mbar_arrive(&full[st]);
+                    break;
+                }
+                const long long base = tk * kTile;
+                s_tile[st] = tk;
+                s_q0[st] = base / L;
+                s_r0[st] = base % L;
+                const long long left = total - base;
+                const unsigned bytes =
+                    static_cast<unsigned>(left < kTile ? left : kTile) * sizeof(T);
+                unsigned char* dst = smem_raw + st * S::kStageBytes;
+                mbar_arrive_expect_tx(&full[st], 2u * bytes);
+                tma_bulk_g2s(dst, a + base, bytes, &full[st]);
+                tma_bulk_g2s(dst + S::kArrayBytes, u + base, bytes, &full[st]);
+            }
+        }
+    } else {
+        // ------------------------------------------------------------ consumer warps
+        // state of the tile between its A and B phases
+        Pair p_excl[J], p_tot[J];
+        long long p_tile = -1, p_q0 = 0, p_r0 = 0;
+        int p_st = 0, p_buf = 0;
+        Pair p_agg = identity_pair();  // warp 0 only
+        bool p_self = false;           // warp 0 only
+
+        for (unsigned it = 0;; ++it) {
+            const int st = static_cast<int>(it % STAGES);
+            const int buf = static_cast<int>(it % 3);
+            mbar_wait(&full[st], (it / STAGES) & 1u);
+            const long long tile = s_tile[st];
+            const bool cur = tile >= 0;
+            const long long base = tile * kTile;
+            const long long q0 = s_q0[st], r0 = s_r0[st];
+            Pair c_excl[J], c_tot[J];
+            if (cur) {
+                // ---- A(it): ring -> registers, heads -> reset pairs, A4 + A5
+                const T* sa = reinterpret_cast<const T*>(smem_raw + st * S::kStageBytes);
+                const T* su = sa + kTile;
+                TileRegs<VEC, J> r;
+#pragma unroll
+                for (int j = 0; j < J; ++j) {
+                    const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                    if (base + off < total) {
+                        unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), r.av[j]);
+                        unpack128<T>(*reinterpret_cast<const uint4*>(su + off), r.uv[j]);
+                    } else {  // identity padding (Q3)
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) { r.av[j][k] = 1.0f; r.uv[j][k] = 0.0f; }
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < J; ++j) {
+                    const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                    long long s, t;
+                    seq_pos(q0, r0, off, L, kTile, s, t);
+                    if (t == 0 && base + off < total) {
+                        const float hin = h0 ? __ldg(h0 + s) : 0.0f;
+                        r.uv[j][0] = fmaf(r.av[j][0], hin, r.uv[j][0]);
+                        r.av[j][0] = 0.0f;
+                    }
+                    row_scan(r, j, lane);
+                    c_excl[j] = r.excl[j];
+                    c_tot[j] = r.tot[j];
+                }
+                const Pair wt = warp_total(r);
+                if (lane == 0) s_warp[buf * WARPS + warp] = wt;
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(WARPS * 32) : "memory");
+            Pair c_agg = identity_pair();
+            bool c_self = false;
+            if (warp == 0) {
+                if (cur) {  // A6/A7: CTA aggregate, published before any waiting
+                    const Pair* sw = s_warp + buf * WARPS;
+                    c_agg = sw[0];
+#pragma unroll
+                    for (int w = 1; w < WARPS; ++w) c_agg = compose(sw[w], c_agg);
+                    c_self = lookback_publish(desc, static_cast<unsigned>(tile), tag, c_agg,
+                                              r0 != 0, lane);
+                }
+                if (p_tile >= 0) {  // the only wait: carry into the previous tile
+                    float h_in = 0.0f;
+                    if (p_r0 != 0)
+                        h_in = lookback_wait(desc, static_cast<unsigned>(p_tile), tag, p_agg,
+                                             p_self, lane);
+                    if (lane == 0) *s_hin = h_in;
+                }
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(WARPS * 32) : "memory");
+            if (p_tile >= 0) {
+                // ---- B(it-1): apply the prefix, rescan from the ring slot, store h, h_last
+                const Pair* sw = s_warp + p_buf * WARPS;
+                Pair X = identity_pair();
+                for (int w = 0; w < warp; ++w) X = compose(sw[w], X);
+                float H = apply(X, *s_hin);
+                const long long pbase = p_tile * kTile;
+                const T* sa = reinterpret_cast<const T*>(smem_raw + p_st * S::kStageBytes);
+                const T* su = sa + kTile;
+#pragma unroll
+                for (int j = 0; j < J; ++j) {
+                    const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                    if (pbase + off < total) {
+                        float av[VEC], uv[VEC];
+                        unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), av);
+                        unpack128<T>(*reinterpret_cast<const uint4*>(su + off), uv);
+                        long long s, t;
+                        seq_pos(p_q0, p_r0, off, L, kTile, s, t);
+                        float hs = apply(p_excl[j], H);
+                        if (t == 0) {  // sequence head: the reset pair (0, a0*h0 + u0)
+                            hs = h0 ? __ldg(h0 + s) : 0.0f;
+                        }
+                        float out[VEC];
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            hs = fmaf(av[k], hs, uv[k]);
+                            out[k] = hs;
+                        }
+                        Acc::store(h + pbase + off, out);
+                        if (h_last && t + VEC == L) h_last[s] = hs;
+                    }
+                    H = apply(p_tot[j], H);
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[p_st]);  // the slot may be refilled
+            }
+            if (!cur) break;
+#pragma unroll
+            for (int j = 0; j < J; ++j) { p_excl[j] = c_excl[j]; p_tot[j] = c_tot[j]; }
+            p_tile = tile; p_q0 = q0; p_r0 = r0; p_st = st; p_buf = buf;
+            p_agg = c_agg; p_self = c_self;
+        }
+    }
+    // The last CTA to exit re-arms the control block for the next launch on this buffer.
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(&ctrl->done, 1u) == gridDim.x - 1) {
             ctrl->ticket = 0;
             ctrl->done = 0;
             ctrl->epoch = tag;  // = old epoch + 1 (mod 2^30)

@@ -37,9 +37,24 @@ int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float*
                            sizeof(LookbackCtrl) + static_cast<size_t>(ntiles) * 16, &sc));
     auto* ctrl = static_cast<LookbackCtrl*>(sc.ptr);
     auto* desc = reinterpret_cast<unsigned long long*>(ctrl + 1);
-    affine_scan_lookback_kernel<T, VEC, kJ, kAffLookbackWarps>
-        <<<static_cast<unsigned>(ntiles), kAffLookbackWarps * 32, 0, stream>>>(
-            a, u, h0, h, h_last, total, L, desc, ctrl);
+    if constexpr (VEC > 1) {
+        // vector path: persistent CTAs, a/u tiles streamed through a TMA ring (affine_scan.cuh)
+        constexpr int kStages = VEC == 8 ? 4 : 3;
+        constexpr int kCtasPerSm = 2;
+        using S = ChainSmem<T, VEC, kJ, kAffLookbackWarps, kStages>;
+        auto kern = affine_scan_chain_kernel<T, VEC, kJ, kAffLookbackWarps, kStages, kCtasPerSm>;
+        AS_TRY(allow_dynamic_smem(reinterpret_cast<const void*>(kern), S::kBytes));
+        int sms = 0;
+        AS_TRY(sm_count(&sms));
+        const int64_t resident = static_cast<int64_t>(sms) * kCtasPerSm;
+        const unsigned grid = static_cast<unsigned>(ntiles < resident ? ntiles : resident);
+        kern<<<grid, (kAffLookbackWarps + 1) * 32, S::kBytes, stream>>>(
+            a, u, h0, h, h_last, total, L, ntiles, desc, ctrl);
+    } else {
+        affine_scan_lookback_kernel<T, VEC, kJ, kAffLookbackWarps>
+            <<<static_cast<unsigned>(ntiles), kAffLookbackWarps * 32, 0, stream>>>(
+                a, u, h0, h, h_last, total, L, desc, ctrl);
+    }
     const int st = after_launch();
     const int st2 = scratch_release(stream, sc);
     return st != AFFINESCAN_OK ? st : st2;

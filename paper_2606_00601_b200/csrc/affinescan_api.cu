@@ -66,6 +66,25 @@ int sm_count(int* out)
     return AFFINESCAN_OK;
 }
 
+namespace {
+std::mutex g_attr_mu;
+std::map<std::pair<const void*, int>, int> g_attr_done;
+}  // namespace
+
+int allow_dynamic_smem(const void* kernel, int bytes)
+{
+    int dev = 0;
+    AS_CUDA(cudaGetDevice(&dev));
+    const std::pair<const void*, int> key{kernel, dev};
+    std::lock_guard<std::mutex> lk(g_attr_mu);
+    auto it = g_attr_done.find(key);
+    if (it == g_attr_done.end() || it->second < bytes) {
+        AS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+        g_attr_done[key] = bytes;
+    }
+    return AFFINESCAN_OK;
+}
+
 int scratch_acquire(cudaStream_t stream, int slot, size_t bytes, Scratch* out)
 {
     *out = Scratch{};

@@ -101,25 +101,10 @@ int make_bc_tensor_map(CUtensorMap* map, const T* base, int64_t rows, int64_t L,
     return AFFINESCAN_OK;
 }
 
-// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (kernel, device).  Keyed by the
-// kernel's address: instantiations share one function-pointer TYPE, so a static per template
-// instantiation of this helper would be shared by all of them.
-std::mutex g_attr_mu;
-std::map<std::pair<const void*, int>, int> g_attr_done;
-
 template <typename Kern>
 int allow_smem(Kern kern, int bytes)
 {
-    int dev = 0;
-    AS_CUDA(cudaGetDevice(&dev));
-    const std::pair<const void*, int> key{reinterpret_cast<const void*>(kern), dev};
-    std::lock_guard<std::mutex> lk(g_attr_mu);
-    auto it = g_attr_done.find(key);
-    if (it == g_attr_done.end() || it->second < bytes) {
-        AS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
-        g_attr_done[key] = bytes;
-    }
-    return AFFINESCAN_OK;
+    return allow_dynamic_smem(reinterpret_cast<const void*>(kern), bytes);
 }
 
 // ---------------------------------------------------------------- typed view of the arguments

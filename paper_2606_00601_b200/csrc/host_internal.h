@@ -37,6 +37,10 @@ inline bool mul_overflows(int64_t a, int64_t b, int64_t* out)
 // ---- device facts (queried once per device)
 int sm_count(int* out);          // cudaDevAttrMultiProcessorCount of the current device
 
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) once per (kernel, device); keyed by the
+// kernel's address.
+int allow_dynamic_smem(const void* kernel, int bytes);
+
 // ---- library-owned device scratch, stream-ordered.
 // Outside stream capture: one cached buffer per (device, stream, slot) that only grows; growing
 // frees the old buffer with cudaFreeAsync and allocates with cudaMallocAsync ON THE CALLER'S

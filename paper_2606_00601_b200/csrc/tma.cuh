@@ -69,6 +69,16 @@ __device__ __forceinline__ void tma_tile_2d_g2s(void* dst_smem, const CUtensorMa
         ::"r"(smem_u32(dst_smem)), "l"(map), "r"(c0), "r"(c1), "r"(smem_u32(bar))
         : "memory");
 }
+// TMA 1-D bulk copy global -> shared (cp.async.bulk; SASS: UBLKCP): `bytes` is a multiple of 16,
+// both addresses 16-byte aligned; completion is counted on the mbarrier in bytes.
+__device__ __forceinline__ void tma_bulk_g2s(void* dst_smem, const void* src, unsigned bytes,
+                                             uint64_t* bar)
+{
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+        ::"r"(smem_u32(dst_smem)), "l"(src), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async_smem()
 {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");

@@ -321,7 +321,7 @@ AFFINESCAN_API int affinescan_version(void);
 /* Tuning knobs for ablations and sweeps (process-wide; -1 restores the default chosen from
  * the shape).  Returns AFFINESCAN_ERR_UNSUPPORTED for an unknown key or value. */
 typedef enum affinescan_option {
-    AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lanes per (b,d) row in the lane_row schedule: 1, 2   */
+    AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lane_row grid: 1 or 2 lanes per (b,d) row; 3 = balanced mix */
     AFFINESCAN_OPT_LANE_ROW_POLY16 = 2  /* sixteenths (0 or 4) of the exponentials evaluated by
                                            the fma-pipe polynomial instead of MUFU.EX2           */
 } affinescan_option;

@@ -453,30 +453,53 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
                 const T* sa = reinterpret_cast<const T*>(smem_raw + st * S::kStageBytes);
                 const T* su = sa + kTile;
                 TileRegs<VEC, J> r;
+                // interior tile (the common case): whole tile inside one sequence and inside the
+                // stream, so a head can only sit at offset 0 and a tail at the tile's end
+                const bool fast = (r0 + kTile <= L) && (base + kTile <= total);
+                if (fast) {
 #pragma unroll
-                for (int j = 0; j < J; ++j) {
-                    const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
-                    if (base + off < total) {
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
                         unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), r.av[j]);
                         unpack128<T>(*reinterpret_cast<const uint4*>(su + off), r.uv[j]);
-                    } else {  // identity padding (Q3)
-#pragma unroll
-                        for (int k = 0; k < VEC; ++k) { r.av[j][k] = 1.0f; r.uv[j][k] = 0.0f; }
                     }
-                }
-#pragma unroll
-                for (int j = 0; j < J; ++j) {
-                    const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
-                    long long s, t;
-                    seq_pos(q0, r0, off, L, kTile, s, t);
-                    if (t == 0 && base + off < total) {
-                        const float hin = h0 ? __ldg(h0 + s) : 0.0f;
-                        r.uv[j][0] = fmaf(r.av[j][0], hin, r.uv[j][0]);
-                        r.av[j][0] = 0.0f;
+                    if (r0 == 0 && threadIdx.x == 0) {
+                        const float hin = h0 ? __ldg(h0 + q0) : 0.0f;
+                        r.uv[0][0] = fmaf(r.av[0][0], hin, r.uv[0][0]);
+                        r.av[0][0] = 0.0f;
                     }
-                    row_scan(r, j, lane);
-                    c_excl[j] = r.excl[j];
-                    c_tot[j] = r.tot[j];
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        row_scan(r, j, lane);
+                        c_excl[j] = r.excl[j];
+                        c_tot[j] = r.tot[j];
+                    }
+                } else {
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                        if (base + off < total) {
+                            unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), r.av[j]);
+                            unpack128<T>(*reinterpret_cast<const uint4*>(su + off), r.uv[j]);
+                        } else {  // identity padding (Q3)
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k) { r.av[j][k] = 1.0f; r.uv[j][k] = 0.0f; }
+                        }
+                    }
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                        long long s, t;
+                        seq_pos(q0, r0, off, L, kTile, s, t);
+                        if (t == 0 && base + off < total) {
+                            const float hin = h0 ? __ldg(h0 + s) : 0.0f;
+                            r.uv[j][0] = fmaf(r.av[j][0], hin, r.uv[j][0]);
+                            r.av[j][0] = 0.0f;
+                        }
+                        row_scan(r, j, lane);
+                        c_excl[j] = r.excl[j];
+                        c_tot[j] = r.tot[j];
+                    }
                 }
                 const Pair wt = warp_total(r);
                 if (lane == 0) s_warp[buf * WARPS + warp] = wt;
@@ -511,19 +534,17 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
                 const long long pbase = p_tile * kTile;
                 const T* sa = reinterpret_cast<const T*>(smem_raw + p_st * S::kStageBytes);
                 const T* su = sa + kTile;
+                const bool fast = (p_r0 + kTile <= L) && (pbase + kTile <= total);
+                if (fast) {
+                    const bool tail = (p_r0 + kTile == L);
 #pragma unroll
-                for (int j = 0; j < J; ++j) {
-                    const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
-                    if (pbase + off < total) {
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
                         float av[VEC], uv[VEC];
                         unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), av);
                         unpack128<T>(*reinterpret_cast<const uint4*>(su + off), uv);
-                        long long s, t;
-                        seq_pos(p_q0, p_r0, off, L, kTile, s, t);
                         float hs = apply(p_excl[j], H);
-                        if (t == 0) {  // sequence head: the reset pair (0, a0*h0 + u0)
-                            hs = h0 ? __ldg(h0 + s) : 0.0f;
-                        }
+                        if (j == 0 && p_r0 == 0 && threadIdx.x == 0) hs = h0 ? __ldg(h0 + p_q0) : 0.0f;
                         float out[VEC];
 #pragma unroll
                         for (int k = 0; k < VEC; ++k) {
@@ -531,9 +552,33 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
                             out[k] = hs;
                         }
                         Acc::store(h + pbase + off, out);
-                        if (h_last && t + VEC == L) h_last[s] = hs;
+                        if (j == J - 1 && tail && h_last && threadIdx.x == WARPS * 32 - 1)
+                            h_last[p_q0] = hs;
+                        H = apply(p_tot[j], H);
                     }
-                    H = apply(p_tot[j], H);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                        if (pbase + off < total) {
+                            float av[VEC], uv[VEC];
+                            unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), av);
+                            unpack128<T>(*reinterpret_cast<const uint4*>(su + off), uv);
+                            long long s, t;
+                            seq_pos(p_q0, p_r0, off, L, kTile, s, t);
+                            float hs = apply(p_excl[j], H);
+                            if (t == 0) hs = h0 ? __ldg(h0 + s) : 0.0f;  // head: the reset pair
+                            float out[VEC];
+#pragma unroll
+                            for (int k = 0; k < VEC; ++k) {
+                                hs = fmaf(av[k], hs, uv[k]);
+                                out[k] = hs;
+                            }
+                            Acc::store(h + pbase + off, out);
+                            if (h_last && t + VEC == L) h_last[s] = hs;
+                        }
+                        H = apply(p_tot[j], H);
+                    }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[p_st]);  // the slot may be refilled

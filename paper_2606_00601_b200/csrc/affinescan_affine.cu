@@ -24,8 +24,9 @@ template <typename T, int VEC>
 int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float* h_last,
                            int64_t num_seq, int64_t L, cudaStream_t stream)
 {
-    // 4096-element tiles for both io dtypes (64 B of a and of u per thread fit 64 registers)
-    constexpr int kJ = VEC == 8 ? kAffLookbackJ / 2 : kAffLookbackJ;
+    // four 128-bit vectors of a and of u per thread: tiles of 4096 (fp32) / 8192 (bf16) elements;
+    // the scalar-access fallback keeps 4096-element tiles
+    constexpr int kJ = kAffLookbackJ;
     constexpr int kTile = kAffLookbackWarps * 32 * VEC * kJ;
     const int64_t total = num_seq * L;
     const int64_t ntiles = (total + kTile - 1) / kTile;
@@ -38,8 +39,9 @@ int launch_affine_lookback(const T* a, const T* u, const float* h0, T* h, float*
     auto* ctrl = static_cast<LookbackCtrl*>(sc.ptr);
     auto* desc = reinterpret_cast<unsigned long long*>(ctrl + 1);
     if constexpr (VEC > 1) {
-        // vector path: persistent CTAs, a/u tiles streamed through a TMA ring (affine_scan.cuh)
-        constexpr int kStages = VEC == 8 ? 4 : 3;
+        // vector path: persistent CTAs, a/u tiles streamed through a TMA ring (affine_scan.cuh);
+        // 3 stages of 32 KB, two CTAs per SM
+        constexpr int kStages = 3;
         constexpr int kCtasPerSm = 2;
         using S = ChainSmem<T, VEC, kJ, kAffLookbackWarps, kStages>;
         auto kern = affine_scan_chain_kernel<T, VEC, kJ, kAffLookbackWarps, kStages, kCtasPerSm>;
@@ -111,7 +113,8 @@ int affine_dispatch(const void* a_, const void* u_, const float* h0, void* h_, f
     if (variant == AFFINESCAN_VARIANT_AUTO) {
         int sms = 0;
         AS_TRY(sm_count(&sms));
-        const int64_t cta_loop_min_seq = static_cast<int64_t>(sms) * 4;   // >= 4 CTAs of 8 warps / SM
+        const int64_t cta_loop_min_seq = static_cast<int64_t>(sms) * 16;  // >= 4 waves of 4 CTAs / SM:
+                                                                          // fewer leave a ragged last wave
         const int64_t warp_seq_min_seq = static_cast<int64_t>(sms) * 64;  // >= 64 warps / SM
         if (num_seq >= cta_loop_min_seq && L >= kAffCtaLoopMinL)
             variant = AFFINESCAN_AFFINE_CTA_LOOP;

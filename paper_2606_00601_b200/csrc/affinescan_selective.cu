@@ -25,7 +25,6 @@ constexpr int64_t kChunkedMinL = 8192;    // chunked (look-back) schedule: at le
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
 constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
 constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
-constexpr int kLaneRowDefaultG = 1;       // lanes per row (r01b sweep: profiles/)
 constexpr int kLaneRowDefaultPoly16 = 4;  // sixteenths of the exps done on the fma pipe
 
 // Tuning knobs of the lane_row schedule (affinescan_set_option); -1 = choose from the shape.
@@ -168,23 +167,43 @@ int launch_warp_row(const Typed<T>& t, bool vec_ok, cudaStream_t stream)
 }
 
 // ---------------------------------------------------------------- lane_row (many rows)
-template <typename T, int G, int F16, int EXT, int ASTR>
+template <typename T, int G, int F16, int EXT, int ASTR, int ORDER = 0, int WARPS = kLaneRowWarps>
 int launch_lane_row_inst(const Typed<T>& t, cudaStream_t stream)
 {
     // polynomial degree per io dtype: DESIGN.md §7 (tolerance argument)
     constexpr int kDeg = sizeof(T) == 2 ? 3 : 5;
     using S = LaneRowSmem<T, kLaneRowTc>;
-    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, kLaneRowWarps, F16, kDeg, EXT, ASTR>;
-    constexpr int smem = S::kPerWarp * kLaneRowWarps;
+    auto kern = selective_scan_lane_row_kernel<T, G, kLaneRowTc, WARPS, F16, kDeg, EXT, ASTR, ORDER>;
+    constexpr int smem = S::kPerWarp * WARPS;
     AS_TRY(allow_smem(kern, smem));
     CUtensorMap mapB, mapC;
     AS_TRY(make_bc_tensor_map<T>(&mapB, t.B, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
     AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
     const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
     const int64_t warps = rows / (32 / G);
-    const int64_t blocks = (warps + kLaneRowWarps - 1) / kLaneRowWarps;
+    const int64_t blocks = (warps + WARPS - 1) / WARPS;
     if (blocks > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
-    kern<<<static_cast<unsigned>(blocks), kLaneRowWarps * 32, smem, stream>>>(
+    kern<<<static_cast<unsigned>(blocks), WARPS * 32, smem, stream>>>(
+        t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner, t.L);
+    return after_launch();
+}
+
+template <typename T, int F16, int EXT, int ORDER>
+int launch_lane_mix_inst(const Typed<T>& t, cudaStream_t stream)
+{
+    constexpr int kDeg = sizeof(T) == 2 ? 3 : 5;
+    using M = LaneMixSmem<T, kLaneRowTc>;
+    auto kern = selective_scan_lane_mix_kernel<T, kLaneRowTc, F16, kDeg, EXT, ORDER>;
+    constexpr int smem = M::kBytes;
+    // a CTA's 224 consecutive rows must lie in at most kMixMaxBatches batches
+    if (t.d_inner < 224 || t.d_inner % 32 != 0) return AFFINESCAN_ERR_UNSUPPORTED;
+    AS_TRY(allow_smem(kern, smem));
+    CUtensorMap mapB, mapC;
+    AS_TRY(make_bc_tensor_map<T>(&mapB, t.B, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
+    AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
+    int sms = 0;
+    AS_TRY(sm_count(&sms));
+    kern<<<static_cast<unsigned>(sms), 17 * 32, smem, stream>>>(
         t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner, t.L);
     return after_launch();
 }
@@ -200,9 +219,11 @@ bool is_gated(const Typed<T>& t)
 template <typename T, int G, int F16>
 int launch_lane_row_gf(const Typed<T>& t, cudaStream_t stream)
 {
-    if (!t.has_ext) return launch_lane_row_inst<T, G, F16, 0, 0>(t, stream);
-    if (G == 1 && is_gated(t)) return launch_lane_row_inst<T, 1, F16, kExtGated, 0>(t, stream);
-    return launch_lane_row_inst<T, G, F16, kExtGeneric, 0>(t, stream);
+    // G = 1 (one or two warps per sub-partition): pass-major; G = 2: timestep-major
+    constexpr int kOrder = G == 1 ? 0 : 1;
+    if (!t.has_ext) return launch_lane_row_inst<T, G, F16, 0, 0, kOrder>(t, stream);
+    if (G == 1 && is_gated(t)) return launch_lane_row_inst<T, 1, F16, kExtGated, 0, 0>(t, stream);
+    return launch_lane_row_inst<T, G, F16, kExtGeneric, 0, kOrder>(t, stream);
 }
 
 template <typename T>
@@ -216,8 +237,27 @@ int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
                          : launch_lane_row_inst<T, 1, 0, 0, 2>(t, stream);
     int G = g_opt_lane_row_g.load(std::memory_order_relaxed);
     int poly16 = g_opt_lane_row_poly16.load(std::memory_order_relaxed);
-    if (G < 0) G = kLaneRowDefaultG;
+    if (G < 0) {
+        // Grid shape from the row count: cycles per timestep on the busiest
+        // sub-partition, fitted to measurements on B200 (w = resident row warps there).
+        int sms = 0;
+        AS_TRY(sm_count(&sms));
+        const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
+        const int64_t smsp = static_cast<int64_t>(sms) * 4;
+        const int64_t w1 = (rows / 32 + smsp - 1) / smsp, w2 = (rows / 16 + smsp - 1) / smsp;
+        const int64_t rounds = (rows + static_cast<int64_t>(sms) * 224 - 1) / (static_cast<int64_t>(sms) * 224);
+        const int64_t c1 = 110 + 118 * w1, c2 = 140 + 59 * w2, c3 = 296 * rounds;
+        const bool mix_ok = t.d_inner >= 224;
+        G = (mix_ok && c3 < c1 && c3 < c2) ? 3 : (c2 < c1 ? 2 : 1);
+        if (poly16 < 0) poly16 = G == 1 ? kLaneRowDefaultPoly16 : 0;
+    }
     if (poly16 < 0) poly16 = kLaneRowDefaultPoly16;
+    if (G == 3) {   // balanced grid: three G = 2 warps + one G = 4 warp per sub-partition
+        if (t.d_inner < 224) return AFFINESCAN_ERR_UNSUPPORTED;
+        if (!t.has_ext) return launch_lane_mix_inst<T, 0, 0, 1>(t, stream);
+        if (is_gated(t)) return launch_lane_mix_inst<T, 0, kExtGated, 1>(t, stream);
+        return launch_lane_mix_inst<T, 0, kExtGeneric, 1>(t, stream);
+    }
     if (G == 1 && poly16 == 0) return launch_lane_row_gf<T, 1, 0>(t, stream);
     if (G == 1 && poly16 == 4) return launch_lane_row_gf<T, 1, 4>(t, stream);
     if (G == 2 && poly16 == 0) return launch_lane_row_gf<T, 2, 0>(t, stream);
@@ -460,7 +500,7 @@ int set_lane_row_option(int key, int value)
 {
     switch (key) {
     case AFFINESCAN_OPT_LANE_ROW_G:
-        if (value != -1 && value != 1 && value != 2) return AFFINESCAN_ERR_UNSUPPORTED;
+        if (value != -1 && (value < 1 || value > 3)) return AFFINESCAN_ERR_UNSUPPORTED;
         g_opt_lane_row_g.store(value);
         return AFFINESCAN_OK;
     case AFFINESCAN_OPT_LANE_ROW_POLY16:

@@ -139,22 +139,35 @@ struct RowSeg<__nv_bfloat16, 2> {
 // WARPS = warps per CTA; F16 = sixteenths of the exponentials done by the polynomial;
 // DEG = its degree; EXT / ASTR: see the header comment.
 // ====================================================================================
-template <typename T, int G, int TC, int WARPS, int F16, int DEG, int EXT, int ASTR>
-__global__ void __launch_bounds__(WARPS * 32)
-selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
-                               const float* __restrict__ A,
-                               const __grid_constant__ CUtensorMap mapB,
-                               const __grid_constant__ CUtensorMap mapC,
-                               const float* __restrict__ D,
-                               const float* __restrict__ h0, T* __restrict__ y,
-                               float* __restrict__ h_last, const SelectiveExt ext, int batch,
-                               int d_inner, long long L)
+// CTA-shared B/C tiles (lane_mix kernel): a producer warp stages the fp32 [TC][2][N] tiles of the
+// batches the CTA touches into a ring of kStages slots; consumers wait on full[slot] and arrive
+// on empty[slot] once per tile.
+constexpr int kMixStages = 3;
+constexpr int kMixMaxBatches = 2;
+struct SharedTiles {
+    const float* bc;   // [kMixStages][kMixMaxBatches][TC][2][N]
+    uint64_t* full;    // [kMixStages], count 1 (producer)
+    uint64_t* empty;   // [kMixStages], count = consumer warps with work
+    int bsel;          // which of the CTA's batches this warp's rows belong to
+};
+
+// The work of ONE warp: RW = 32/G consecutive rows starting at row0 (all in one batch), walked
+// over the whole of L.  SHARED == false: `wbase` is the warp's private
+// LaneRowSmem<T, TC>::kPerWarp bytes and the warp stages its own B/C tiles; SHARED == true: the
+// tiles come from `sh`.
+template <typename T, int G, int TC, int F16, int DEG, int EXT, int ASTR, int ORDER,
+          bool SHARED = false>
+__device__ __forceinline__ void
+lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float* __restrict__ A,
+              const CUtensorMap* mapB, const CUtensorMap* mapC, const float* __restrict__ D,
+              const float* __restrict__ h0, T* __restrict__ y, float* __restrict__ h_last,
+              const SelectiveExt& ext, int d_inner, long long L, long long row0,
+              unsigned char* wbase, const SharedTiles sh = SharedTiles{})
 {
     using S = LaneRowSmem<T, TC>;
     constexpr int N = S::N;
     constexpr int VEC = Io<T>::kVec;   // timesteps per 128-bit access
     constexpr int kChunks = TC / VEC;  // 128-bit chunks per raw row
-    constexpr int RW = 32 / G;         // rows per warp
     constexpr int NS = N / G;          // states per lane
     constexpr int NP = NS / 2;         // packed pairs per lane
     constexpr int PP = 2;              // packed pairs per pass (four states share a MUFU burst)
@@ -164,40 +177,38 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     static_assert(NS % 4 == 0 && YC >= 1 && TC % VEC == 0 && (TC / VEC) % 2 == 0, "shape");
     static_assert(ASTR == 0 || (G == 1 && F16 == 0), "structured-A paths: one lane per row, no polynomial");
 
-    extern __shared__ __align__(128) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
     const int g = lane % G;  // which NS-slice of the row's states
-    const long long rows = static_cast<long long>(batch) * d_inner;
-    const long long row0 = (static_cast<long long>(blockIdx.x) * WARPS + warp) * RW;
-    if (row0 >= rows) return;  // whole warp exits together; warps never sync with each other
     const long long row = row0 + lane / G;
-    const int b = static_cast<int>(row0 / d_inner);  // d_inner % 32 == 0: uniform over the warp
+    const int b = static_cast<int>(row0 / d_inner);  // d_inner % (32/G) == 0: uniform over the warp
     const int d = static_cast<int>(row - static_cast<long long>(b) * d_inner);
 
-    unsigned char* wbase = smem_raw + static_cast<size_t>(warp) * S::kPerWarp;
-    float* bc = reinterpret_cast<float*>(wbase + 2 * S::kRawStage);
-    uint64_t* full = reinterpret_cast<uint64_t*>(wbase + 2 * S::kRawStage + S::kBcTile);
+    const float* bc = SHARED ? sh.bc : reinterpret_cast<const float*>(wbase + 2 * S::kRawStage);
+    float* bcw = SHARED ? nullptr : reinterpret_cast<float*>(wbase + 2 * S::kRawStage);
+    uint64_t* full =
+        SHARED ? sh.full : reinterpret_cast<uint64_t*>(wbase + 2 * S::kRawStage + S::kBcTile);
 
-    if (lane == 0) {
-        mbar_init(&full[0], 1);
-        mbar_init(&full[1], 1);
-        fence_mbar_init();
+    if (!SHARED) {
+        if (lane == 0) {
+            mbar_init(&full[0], 1);
+            mbar_init(&full[1], 1);
+            fence_mbar_init();
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
     }
-    fence_proxy_async_smem();
-    __syncwarp();
 
     const long long ntiles = (L + TC - 1) / TC;
     // A2 staging: one elected lane issues two tensor copies per tile: box {TC, N} of B[b] and
     // of C[b] (tensor maps over [batch*N, L]); the tail tile is zero-filled by the TMA unit.
     auto issue_tile = [&](long long tile) {
-        if (lane == 0) {
+        if (!SHARED && lane == 0) {
             const int st = static_cast<int>(tile & 1);
             const int t0 = static_cast<int>(tile * TC);
             unsigned char* dst = wbase + st * S::kRawStage;
             mbar_arrive_expect_tx(&full[st], static_cast<unsigned>(S::kRawStage));
-            tma_tile_2d_g2s(dst, &mapB, t0, b * N, &full[st]);
-            tma_tile_2d_g2s(dst + N * S::kRawPitch, &mapC, t0, b * N, &full[st]);
+            tma_tile_2d_g2s(dst, mapB, t0, b * N, &full[st]);
+            tma_tile_2d_g2s(dst + N * S::kRawPitch, mapC, t0, b * N, &full[st]);
         }
     };
     issue_tile(0);
@@ -222,7 +233,7 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     if (ASTR != 0) A20 = __ldg(A + static_cast<long long>(d) * N) * kLog2e;
     // the polynomial is used only while |delta*A2| <= 126 for every state of the lane
     const float dmax = 126.0f / (amax * kLog2e);
-    const float Dg = (D && g == 0) ? __ldg(D + d) : 0.0f;  // the skip term is added by one lane
+    const float Dg = D ? __ldg(D + d) : 0.0f;  // skip term, added after the reduction over n
     constexpr bool kRt = (EXT & kExtRuntime) != 0;
     const float bias = ((EXT & kExtSoftplus) && ext.delta_bias) ? __ldg(ext.delta_bias + d) : 0.0f;
 
@@ -252,25 +263,32 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
     }
 
     for (long long tile = 0; tile < ntiles; ++tile) {
-        const int st = static_cast<int>(tile & 1);
-        const unsigned parity = static_cast<unsigned>((tile >> 1) & 1);
         const long long t0 = tile * TC;
-        mbar_wait(&full[st], parity);
-        __syncwarp();  // every lane is done reading the fp32 tile of the previous iteration
-        // A2: widen + transpose raw [2N][TC] (io dtype) -> bc [TC][2][N] (fp32); the
-        // transposed stores hit 32 distinct banks.
+        int slot = 0;
+        if (SHARED) {
+            slot = static_cast<int>(tile % kMixStages);
+            mbar_wait(&full[slot], static_cast<unsigned>((tile / kMixStages) & 1));
+            bc = sh.bc + (slot * kMixMaxBatches + sh.bsel) * (TC * 2 * N);
+        } else {
+            const int st = static_cast<int>(tile & 1);
+            const unsigned parity = static_cast<unsigned>((tile >> 1) & 1);
+            mbar_wait(&full[st], parity);
+            __syncwarp();  // every lane is done reading the fp32 tile of the previous iteration
+            // A2: widen + transpose raw [2N][TC] (io dtype) -> bc [TC][2][N] (fp32); the
+            // transposed stores hit 32 distinct banks.
 #pragma unroll
-        for (int c = 0; c < kChunks; ++c) {
-            float v[VEC];
-            unpack128<T>(*reinterpret_cast<const uint4*>(wbase + st * S::kRawStage +
-                                                         lane * S::kRawPitch + c * 16), v);
+            for (int c = 0; c < kChunks; ++c) {
+                float v[VEC];
+                unpack128<T>(*reinterpret_cast<const uint4*>(wbase + st * S::kRawStage +
+                                                             lane * S::kRawPitch + c * 16), v);
 #pragma unroll
-            for (int k = 0; k < VEC; ++k) bc[(c * VEC + k) * 2 * N + lane] = v[k];
-        }
-        __syncwarp();
-        if (tile + 2 < ntiles) {
-            fence_proxy_async_smem();  // generic reads of the raw stage before the async overwrite
-            issue_tile(tile + 2);
+                for (int k = 0; k < VEC; ++k) bcw[(c * VEC + k) * 2 * N + lane] = v[k];
+            }
+            __syncwarp();
+            if (tile + 2 < ntiles) {
+                fence_proxy_async_smem();  // generic reads of the raw stage before the async overwrite
+                issue_tile(tile + 2);
+            }
         }
 
         // A3..A9: sequential in t
@@ -310,7 +328,6 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 #pragma unroll
                     for (int k = 0; k < VEC; ++k) {
                         dxs[k] = dl[k] * xv[k];
-                        y2[k] = pk(Dg * xv[k], 0.0f);
                     }
                     // structured A: the decay base r_k = 2^(delta_k A2[d,0]) of each timestep
                     pair_t cur[ASTR == 2 ? VEC : 1];
@@ -369,7 +386,49 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                                     *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
                                 h2[p] = fma2(av[k][s], h2[p], mul2(dxx, b4.x));
                                 h2[p + 1] = fma2(av[k][s + 1], h2[p + 1], mul2(dxx, b4.y));
-                                y2[k] = fma2(c4.x, h2[p], y2[k]);
+                                y2[k] = p == 0 ? mul2(c4.x, h2[p]) : fma2(c4.x, h2[p], y2[k]);
+                                y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
+                            }
+                        }
+                    };
+                    // ORDER == 1: timestep-major.  All the states of a lane for one timestep, then
+                    // the next timestep: the MUFU, fma-pipe and LDS instructions of a warp come
+                    // evenly mixed instead of in bursts (a burst of 2^x fills the SMSP's shared
+                    // MIO queue and stalls the other warps' LDS: measured with 4 warps per SMSP).
+                    auto steps = [&](auto ftag, auto rtag) {
+                        constexpr int F = decltype(ftag)::value;
+                        constexpr bool RST = decltype(rtag)::value;
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            const pair_t dd = pk(dl[k], dl[k]);
+                            const pair_t dxx = pk(dxs[k], dxs[k]);
+                            const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS;
+                            const bool rs = RST && ((rmask >> k) & 1u);
+#pragma unroll
+                            for (int p = 0; p < NP; p += 2) {
+                                const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 2 * p);
+                                const ulonglong2 c4 =
+                                    *reinterpret_cast<const ulonglong2*>(bct + N + 2 * p);
+                                pair_t a2[2];
+#pragma unroll
+                                for (int s = 0; s < 2; ++s) {
+                                    if (ASTR == 1) {
+                                        a2[s] = pk(r1[k], r1[k]);
+                                    } else if (ASTR == 2) {
+                                        if (p + s > 0) cur[k] = mul2(cur[k], pk(r2[k], r2[k]));
+                                        a2[s] = cur[k];
+                                    } else if (lane_row_slot_is_poly(k * NP + p + s, F)) {
+                                        a2[s] = exp2_poly2<DEG>(dd, A2p[p + s]);
+                                    } else {
+                                        float lo, hi;
+                                        upk(mul2(dd, A2p[p + s]), lo, hi);
+                                        a2[s] = pk(ex2_approx(lo), ex2_approx(hi));
+                                    }
+                                    if (rs) a2[s] = pk(0.0f, 0.0f);
+                                }
+                                h2[p] = fma2(a2[0], h2[p], mul2(dxx, b4.x));
+                                h2[p + 1] = fma2(a2[1], h2[p + 1], mul2(dxx, b4.y));
+                                y2[k] = p == 0 ? mul2(c4.x, h2[p]) : fma2(c4.x, h2[p], y2[k]);
                                 y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
                             }
                         }
@@ -384,7 +443,12 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                         for (int k = 1; k < VEC; ++k) dm = fmaxf(dm, fabsf(dl[k]));
                         poly_ok = !__any_sync(kFullMask, !(dm <= dmax));
                     }
-                    if ((EXT & kExtReset) && rmask != 0) {  // warp-uniform (rows of a warp share b)
+                    if (ORDER == 1) {
+                        if ((EXT & kExtReset) && rmask != 0)
+                            steps(std::integral_constant<int, 0>{}, std::true_type{});
+                        else if (poly_ok) steps(std::integral_constant<int, F16>{}, std::false_type{});
+                        else steps(std::integral_constant<int, 0>{}, std::false_type{});
+                    } else if ((EXT & kExtReset) && rmask != 0) {  // warp-uniform (rows of a warp share b)
 #pragma unroll
                         for (int q = 0; q < NP / PP; ++q)
                             pass(q, std::integral_constant<int, 0>{}, std::true_type{});
@@ -405,6 +469,8 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                     }
                     // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
                     // each lane ends with YC fully reduced timesteps) and store
+                    // (xv follows the same selection: the skip term D x is added to the values
+                    // a lane keeps)
                     if (G >= 2) {
                         const bool up = (g & (G / 2)) != 0;
 #pragma unroll
@@ -412,6 +478,7 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                             const float mine = up ? ys[VEC / 2 + j] : ys[j];
                             const float send = up ? ys[j] : ys[VEC / 2 + j];
                             ys[j] = mine + __shfl_xor_sync(kFullMask, send, G / 2);
+                            xv[j] = up ? xv[VEC / 2 + j] : xv[j];
                         }
                     }
                     if (G >= 4) {
@@ -421,11 +488,12 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                             const float mine = up ? ys[VEC / 4 + j] : ys[j];
                             const float send = up ? ys[j] : ys[VEC / 4 + j];
                             ys[j] = mine + __shfl_xor_sync(kFullMask, send, 1);
+                            xv[j] = up ? xv[VEC / 4 + j] : xv[j];
                         }
                     }
                     float out[YC];
 #pragma unroll
-                    for (int j = 0; j < YC; ++j) out[j] = ys[j];
+                    for (int j = 0; j < YC; ++j) out[j] = fmaf(Dg, xv[j], ys[j]);
                     if ((EXT & kExtGate) && (!kRt || zr)) {  // f1 epilogue: y <- y * silu(z)
 #pragma unroll
                         for (int j = 0; j < YC; ++j) out[j] *= silu_io<T>(zv[j]);
@@ -433,6 +501,10 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
                     if (y) RowSeg<T, YC>::store(yr + tg + yoff, out);  // y == NULL: aggregate-only call
                 }
             }
+        }
+        if (SHARED) {  // this warp is done with the slot
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sh.empty[slot]);
         }
     }
     // A10: final state
@@ -443,6 +515,175 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
             upk(h2[2 * q + 0], a0, a1);
             upk(h2[2 * q + 1], a2, a3);
             reinterpret_cast<float4*>(h_last + row * N + g * NS)[q] = make_float4(a0, a1, a2, a3);
+        }
+    }
+}
+
+// ====================================================================================
+// Uniform grid: every warp of every CTA takes the next 32/G rows.
+// ====================================================================================
+template <typename T, int G, int TC, int WARPS, int F16, int DEG, int EXT, int ASTR, int ORDER = 0>
+__global__ void __launch_bounds__(WARPS * 32)
+selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ delta,
+                               const float* __restrict__ A,
+                               const __grid_constant__ CUtensorMap mapB,
+                               const __grid_constant__ CUtensorMap mapC,
+                               const float* __restrict__ D,
+                               const float* __restrict__ h0, T* __restrict__ y,
+                               float* __restrict__ h_last, const SelectiveExt ext, int batch,
+                               int d_inner, long long L)
+{
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int warp = threadIdx.x >> 5;
+    const long long rows = static_cast<long long>(batch) * d_inner;
+    const long long row0 = (static_cast<long long>(blockIdx.x) * WARPS + warp) * (32 / G);
+    if (row0 >= rows) return;  // whole warp exits together; warps never sync with each other
+    lane_row_warp<T, G, TC, F16, DEG, EXT, ASTR, ORDER>(
+        x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0,
+        smem_raw + static_cast<size_t>(warp) * LaneRowSmem<T, TC>::kPerWarp);
+}
+
+// ====================================================================================
+// Balanced grid (one CTA per SM: 16 row warps + 1 producer warp): the XU pipe of a sub-partition
+// is the wall, and with R rows the uniform grid leaves sub-partitions holding ceil(...) warps
+// next to ones holding floor(...).  Here every sub-partition gets three G = 2 warps (16 rows
+// each) and one G = 4 warp (8 rows): 56 rows = 7/8 of what two G = 1 warps carry, spread over
+// four warps whose MUFU, fma and LDS instructions interleave.  Warp w of a CTA runs on
+// sub-partition w % 4.  CTA c owns rows [224 c, 224 c + 224) of a round (rounds of grid * 224
+// rows): the first 192 go to the G = 2 warps, the last 32 to the G = 4 warps.  Those rows lie in
+// at most kMixMaxBatches batches (the launcher checks d_inner), whose B/C tiles the producer
+// warp stages ONCE for the whole CTA: TMA tensor copies of the raw [2N][TC] boxes into a
+// two-slot raw ring, widened and transposed into a kMixStages-deep ring of fp32 [TC][2][N]
+// tiles that the row warps read with broadcast LDS.128.
+// ====================================================================================
+template <typename T, int TC>
+struct LaneMixSmem {
+    using S = LaneRowSmem<T, TC>;
+    static constexpr int kBcBytes = kMixStages * kMixMaxBatches * S::kBcTile;
+    static constexpr int kRawBytes = 2 * kMixMaxBatches * S::kRawStage;
+    static constexpr int kBarOffset = kBcBytes + kRawBytes;
+    static constexpr int kBytes = kBarOffset + (2 * kMixStages + 2) * 8 + 64;
+};
+
+template <typename T, int TC, int F16, int DEG, int EXT, int ORDER>
+__global__ void __launch_bounds__(17 * 32, 1)
+selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ delta,
+                               const float* __restrict__ A,
+                               const __grid_constant__ CUtensorMap mapB,
+                               const __grid_constant__ CUtensorMap mapC,
+                               const float* __restrict__ D,
+                               const float* __restrict__ h0, T* __restrict__ y,
+                               float* __restrict__ h_last, const SelectiveExt ext, int batch,
+                               int d_inner, long long L)
+{
+    using M = LaneMixSmem<T, TC>;
+    using S = LaneRowSmem<T, TC>;
+    constexpr int N = S::N;
+    constexpr int VEC = Io<T>::kVec;
+    constexpr int kChunks = TC / VEC;
+    constexpr int kRowsPerCta = 12 * 16 + 4 * 8;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    float* bc_ring = reinterpret_cast<float*>(smem_raw);
+    unsigned char* raw_ring = smem_raw + M::kBcBytes;
+    uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + M::kBarOffset);
+    uint64_t* empty = full + kMixStages;
+    uint64_t* raw_full = empty + kMixStages;
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const long long rows = static_cast<long long>(batch) * d_inner;
+    const long long per_round = static_cast<long long>(gridDim.x) * kRowsPerCta;
+    const long long ntiles = (L + TC - 1) / TC;
+
+    for (long long base = 0; base < rows; base += per_round) {
+        const long long cta0 = base + static_cast<long long>(blockIdx.x) * kRowsPerCta;
+        if (cta0 >= rows) break;  // CTA-uniform
+        const long long cta_rows = rows - cta0 < kRowsPerCta ? rows - cta0 : kRowsPerCta;
+        // rows of this CTA: G = 2 warps take 16 each from the front, G = 4 warps 8 each after them
+        const long long r2 = cta_rows < 192 ? (cta_rows / 16) * 16 : 192;
+        const int n2 = static_cast<int>(r2 / 16);
+        const int n4 = static_cast<int>((cta_rows - r2 + 7) / 8);  // <= 4 (cta_rows % 8 == 0)
+        const int b_first = static_cast<int>(cta0 / d_inner);
+        const int nb = static_cast<int>((cta0 + cta_rows - 1) / d_inner) - b_first + 1;
+        __syncthreads();  // previous round's barriers are quiet
+        if (threadIdx.x == 0) {
+            if (base != 0) {
+#pragma unroll
+                for (int s = 0; s < 2 * kMixStages + 2; ++s) mbar_inval(&full[s]);
+            }
+#pragma unroll
+            for (int s = 0; s < kMixStages; ++s) {
+                mbar_init(&full[s], 1);
+                mbar_init(&empty[s], n2 + n4);
+            }
+            mbar_init(&raw_full[0], 1);
+            mbar_init(&raw_full[1], 1);
+            fence_mbar_init();
+        }
+        fence_proxy_async_smem();
+        __syncthreads();
+
+        if (warp == 16) {
+            // ------------------------------------------------------------ producer warp
+            auto issue_raw = [&](long long tile) {
+                if (lane == 0) {
+                    const int rs = static_cast<int>(tile & 1);
+                    const int t0 = static_cast<int>(tile * TC);
+                    mbar_arrive_expect_tx(&raw_full[rs], static_cast<unsigned>(nb * S::kRawStage));
+                    for (int j = 0; j < nb; ++j) {
+                        unsigned char* dst = raw_ring + (rs * kMixMaxBatches + j) * S::kRawStage;
+                        tma_tile_2d_g2s(dst, &mapB, t0, (b_first + j) * N, &raw_full[rs]);
+                        tma_tile_2d_g2s(dst + N * S::kRawPitch, &mapC, t0, (b_first + j) * N,
+                                        &raw_full[rs]);
+                    }
+                }
+            };
+            issue_raw(0);
+            if (ntiles > 1) issue_raw(1);
+            for (long long tile = 0; tile < ntiles; ++tile) {
+                const int slot = static_cast<int>(tile % kMixStages);
+                const int rs = static_cast<int>(tile & 1);
+                if (tile >= kMixStages)
+                    mbar_wait(&empty[slot], static_cast<unsigned>((tile / kMixStages - 1) & 1));
+                mbar_wait(&raw_full[rs], static_cast<unsigned>((tile >> 1) & 1));
+                for (int j = 0; j < nb; ++j) {
+                    const unsigned char* src =
+                        raw_ring + (rs * kMixMaxBatches + j) * S::kRawStage + lane * S::kRawPitch;
+                    float* dst = bc_ring + (slot * kMixMaxBatches + j) * (TC * 2 * N);
+#pragma unroll
+                    for (int c = 0; c < kChunks; ++c) {
+                        float v[VEC];
+                        unpack128<T>(*reinterpret_cast<const uint4*>(src + c * 16), v);
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) dst[(c * VEC + k) * 2 * N + lane] = v[k];
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&full[slot]);
+                if (tile + 2 < ntiles) {
+                    fence_proxy_async_smem();  // generic reads of the raw slot before the async overwrite
+                    issue_raw(tile + 2);
+                }
+            }
+        } else {
+            // ------------------------------------------------------------ row warps
+            SharedTiles sh;
+            sh.bc = bc_ring;
+            sh.full = full;
+            sh.empty = empty;
+            if (warp < 12) {
+                if (warp < n2) {
+                    const long long row0 = cta0 + warp * 16;
+                    sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
+                    lane_row_warp<T, 2, TC, F16, DEG, EXT, 0, ORDER, true>(
+                        x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh);
+                }
+            } else if (warp - 12 < n4) {
+                const long long row0 = cta0 + r2 + (warp - 12) * 8;
+                sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
+                lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true>(
+                    x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh);
+            }
         }
     }
 }

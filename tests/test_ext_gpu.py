@@ -196,6 +196,46 @@ def test_everything_fused_at_once_and_host_entry_point(cuda_device):
         assert_close(hlh, hlref, dtype, f"all-fused host {dtype} h_last")
 
 
+# ----------------------------------------------------------- lane_row balanced grid (mix)
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_lane_row_balanced_grid_partial_ctas_rounds_and_fused_steps(cuda_device, dtype):
+    """OPT_LANE_ROW_G = 3: one CTA per SM, three 16-row warps and one 8-row warp per
+    sub-partition, B/C staged once per CTA by a producer warp.  Shapes: a CTA's 224 rows
+    straddling two batches, a last CTA with fewer rows than warps, more rows than one round of
+    CTAs holds, L not a multiple of the staged tile; plain, gated and reset forms."""
+    sms = torch.cuda.get_device_properties(cuda_device).multi_processor_count
+    vec = 4 if dtype == torch.float32 else 8
+    lib.set_option(lib.OPT_LANE_ROW_G, 3)
+    try:
+        seed = 900
+        for (batch, d_inner, L) in [(1, 224, 64), (3, 256, 3 * 32 + vec), (2, 480, 520),
+                                    (1, 224 * sms + 96, 40), (5, 1024, 96 + vec)]:
+            for mode in ("plain", "gated", "reset"):
+                seed += 1
+                inp = _inputs(batch, d_inner, L, dtype, cuda_device, seed, with_h0=(seed % 2 == 0))
+                z = bias = reset = None
+                softplus = False
+                if mode == "gated":
+                    inp["delta"] = _raw_delta(inp, seed, cuda_device)
+                    z, bias, _ = _ext_extras(inp, seed, cuda_device)
+                    softplus = True
+                elif mode == "reset":
+                    _, _, reset = _ext_extras(inp, seed, cuda_device, False, False,
+                                              resets=[(0, 0), (0, L // 2), (batch - 1, L - 1), (1, 7)])
+                y, hl = gpu_ext(inp, z, bias, reset, softplus, lib.SELECTIVE_LANE_ROW)
+                assert lib.last_variant() == lib.SELECTIVE_LANE_ROW
+                yref, hlref = oracle_ext(inp, z, bias, reset, softplus)
+                what = f"lane_mix {mode} {dtype} {batch}x{d_inner}x{L}"
+                assert_close(y, yref, dtype, what + " y")
+                assert_close(hl, hlref, dtype, what + " h_last")
+        # narrower than one CTA's 224 rows: the balanced grid does not apply
+        inp = _inputs(2, 192, 64, dtype, cuda_device, 7)
+        with pytest.raises(lib.AffineScanError):
+            gpu_ext(inp, None, None, None, False, lib.SELECTIVE_LANE_ROW)
+    finally:
+        lib.set_option(lib.OPT_LANE_ROW_G, -1)
+
+
 # --------------------------------------------------------------- f5: structured-A fast paths
 @pytest.mark.parametrize("dtype", DTYPES)
 @pytest.mark.parametrize("structure", [lib.A_SCALAR_PER_ROW, lib.A_POWERS])

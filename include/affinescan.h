@@ -74,7 +74,8 @@ typedef enum affinescan_dtype {
 typedef enum affinescan_variant {
     AFFINESCAN_VARIANT_AUTO = 0,
     /* affine_scan */
-    AFFINESCAN_AFFINE_LOOKBACK = 1, /* single pass over the flattened [num_seq*L] stream;
+    AFFINESCAN_AFFINE_LOOKBACK = 1, /* single pass over the flattened [num_seq*L] stream by
+                                       persistent CTAs (tiles streamed through a TMA ring);
                                        decoupled look-back carry between tiles; sequence
                                        heads are reset pairs (0, a0*h0+u0)  (BJ)          */
     AFFINESCAN_AFFINE_CTA_LOOP = 2, /* one CTA per sequence, loop over L with the carry in
@@ -91,10 +92,14 @@ typedef enum affinescan_variant {
                                                sharing B_t/C_t tiles staged in shared memory
                                                by TMA tensor copies (needs N == 16, 16-byte
                                                aligned pointers, L a multiple of the vector) */
-    AFFINESCAN_SELECTIVE_LANE_ROW = 12, /* one lane per (b,d) row, sequential in L; B/C tiles
-                                           staged in shared memory by TMA tensor copies
-                                           (needs N == 16, d_inner % 32 == 0, 16-byte aligned
-                                           pointers, L a multiple of the vector)           */
+    AFFINESCAN_SELECTIVE_LANE_ROW = 12, /* 1, 2 or 4 lanes per (b,d) row, sequential in L, the
+                                           row's states in registers; B/C tiles staged in
+                                           shared memory by TMA tensor copies; the grid is
+                                           uniform (one or two lanes per row) or balanced
+                                           (one CTA per SM, every sub-partition three two-lane
+                                           warps and one four-lane warp), chosen from the row
+                                           count (needs N == 16, d_inner % 32 == 0, 16-byte
+                                           aligned pointers, L a multiple of the vector)   */
     AFFINESCAN_SELECTIVE_CHUNKED = 14   /* few rows x long L: L is cut into chunks that run on
                                            different CTAs; the carry h_in crosses chunks by
                                            decoupled look-back over per-(row, state) chunk

@@ -233,7 +233,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
     if (ASTR != 0) A20 = __ldg(A + static_cast<long long>(d) * N) * kLog2e;
     // the polynomial is used only while |delta*A2| <= 126 for every state of the lane
     const float dmax = 126.0f / (amax * kLog2e);
-    const float Dg = D ? __ldg(D + d) : 0.0f;  // skip term, added after the reduction over n
+    const float Dg = (D && g == 0) ? __ldg(D + d) : 0.0f;  // the skip term is added by one lane
     constexpr bool kRt = (EXT & kExtRuntime) != 0;
     const float bias = ((EXT & kExtSoftplus) && ext.delta_bias) ? __ldg(ext.delta_bias + d) : 0.0f;
 
@@ -291,20 +291,23 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
             }
         }
 
-        // A3..A9: sequential in t
-#pragma unroll 1
-        for (int gi = 0; gi < kChunks; gi += PD) {
-#pragma unroll
-            for (int pi = 0; pi < PD; ++pi) {
-                const int grp = gi + pi;
-                const long long tg = t0 + grp * VEC;
-                if (grp < kChunks && tg < L) {  // warp-uniform
+        // A3..A9: sequential in t.  One group = VEC timesteps of the warp's rows.
+        auto group = [&](auto pitag, const int grp, const long long tg) {
+            constexpr int PI = decltype(pitag)::value;
                     float xv[VEC], dl[VEC];
-                    unpack128<T>(xq[pi], xv);
-                    unpack128<T>(dq[pi], dl);
-                    if (tg + PD * VEC < L) {
-                        xq[pi] = __ldcs(reinterpret_cast<const uint4*>(xr + tg + PD * VEC));
-                        dq[pi] = __ldcs(reinterpret_cast<const uint4*>(dr + tg + PD * VEC));
+                    unpack128<T>(xq[PI], xv);
+                    unpack128<T>(dq[PI], dl);
+                    {   // refill the prefetch slot.  G >= 2 (four warps per sub-partition): always,
+                        // past the end of the row this group is re-read and never used (a
+                        // conditional refill costs a register copy per word: +2.5 %); G = 1:
+                        // conditional (measured: the unconditional form is scheduled late and
+                        // the one or two resident warps cannot hide it: 0.355 -> 0.425 ms)
+                        const long long tn = tg + PD * VEC;
+                        const long long ta = (G >= 2 && tn >= L) ? tg : tn;
+                        if (G >= 2 || tn < L) {
+                            xq[PI] = __ldcs(reinterpret_cast<const uint4*>(xr + ta));
+                            dq[PI] = __ldcs(reinterpret_cast<const uint4*>(dr + ta));
+                        }
                     }
                     // f1 prologue: Delta = softplus(delta + bias[d]); f2: reset bits of the group
                     unsigned rmask = 0;
@@ -328,6 +331,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
 #pragma unroll
                     for (int k = 0; k < VEC; ++k) {
                         dxs[k] = dl[k] * xv[k];
+                        y2[k] = pk(Dg * xv[k], 0.0f);
                     }
                     // structured A: the decay base r_k = 2^(delta_k A2[d,0]) of each timestep
                     pair_t cur[ASTR == 2 ? VEC : 1];
@@ -386,7 +390,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                                     *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
                                 h2[p] = fma2(av[k][s], h2[p], mul2(dxx, b4.x));
                                 h2[p + 1] = fma2(av[k][s + 1], h2[p + 1], mul2(dxx, b4.y));
-                                y2[k] = p == 0 ? mul2(c4.x, h2[p]) : fma2(c4.x, h2[p], y2[k]);
+                                y2[k] = fma2(c4.x, h2[p], y2[k]);
                                 y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
                             }
                         }
@@ -428,7 +432,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                                 }
                                 h2[p] = fma2(a2[0], h2[p], mul2(dxx, b4.x));
                                 h2[p + 1] = fma2(a2[1], h2[p + 1], mul2(dxx, b4.y));
-                                y2[k] = p == 0 ? mul2(c4.x, h2[p]) : fma2(c4.x, h2[p], y2[k]);
+                                y2[k] = fma2(c4.x, h2[p], y2[k]);
                                 y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
                             }
                         }
@@ -469,8 +473,6 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                     }
                     // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
                     // each lane ends with YC fully reduced timesteps) and store
-                    // (xv follows the same selection: the skip term D x is added to the values
-                    // a lane keeps)
                     if (G >= 2) {
                         const bool up = (g & (G / 2)) != 0;
 #pragma unroll
@@ -478,7 +480,6 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                             const float mine = up ? ys[VEC / 2 + j] : ys[j];
                             const float send = up ? ys[j] : ys[VEC / 2 + j];
                             ys[j] = mine + __shfl_xor_sync(kFullMask, send, G / 2);
-                            xv[j] = up ? xv[VEC / 2 + j] : xv[j];
                         }
                     }
                     if (G >= 4) {
@@ -488,18 +489,29 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                             const float mine = up ? ys[VEC / 4 + j] : ys[j];
                             const float send = up ? ys[j] : ys[VEC / 4 + j];
                             ys[j] = mine + __shfl_xor_sync(kFullMask, send, 1);
-                            xv[j] = up ? xv[VEC / 4 + j] : xv[j];
                         }
                     }
                     float out[YC];
 #pragma unroll
-                    for (int j = 0; j < YC; ++j) out[j] = fmaf(Dg, xv[j], ys[j]);
+                    for (int j = 0; j < YC; ++j) out[j] = ys[j];
                     if ((EXT & kExtGate) && (!kRt || zr)) {  // f1 epilogue: y <- y * silu(z)
 #pragma unroll
                         for (int j = 0; j < YC; ++j) out[j] *= silu_io<T>(zv[j]);
                     }
                     if (y) RowSeg<T, YC>::store(yr + tg + yoff, out);  // y == NULL: aggregate-only call
-                }
+        };
+        if (G >= 2 && t0 + TC <= L) {  // whole tile inside the row: no per-group conditions
+#pragma unroll 1
+            for (int gi = 0; gi < kChunks; gi += PD) {
+                group(std::integral_constant<int, 0>{}, gi, t0 + gi * VEC);
+                group(std::integral_constant<int, 1>{}, gi + 1, t0 + (gi + 1) * VEC);
+            }
+        } else {
+#pragma unroll 1
+            for (int gi = 0; gi < kChunks; gi += PD) {
+                if (t0 + gi * VEC < L) group(std::integral_constant<int, 0>{}, gi, t0 + gi * VEC);
+                if (t0 + (gi + 1) * VEC < L)
+                    group(std::integral_constant<int, 1>{}, gi + 1, t0 + (gi + 1) * VEC);
             }
         }
         if (SHARED) {  // this warp is done with the slot

@@ -60,7 +60,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
     def compile_one(src):
         obj = os.path.join(objdir, os.path.basename(src) + ".o")
-        cmd = [nvcc, *NVCC_COMPILE_FLAGS, "-I", os.path.join(ROOT, "include"), "-c", "-o", obj, src]
+        cmd = [nvcc, *NVCC_COMPILE_FLAGS, *os.environ.get("AFFINESCAN_NVCC_FLAGS", "").split(),
+               "-I", os.path.join(ROOT, "include"), "-c", "-o", obj, src]
         if verbose:
             cmd[1:1] = ["-Xptxas", "-v"]
             print(" ".join(cmd), file=sys.stderr)

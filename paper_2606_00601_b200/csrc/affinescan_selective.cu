@@ -23,7 +23,10 @@ constexpr int kWarpRowTmaMaxWarps = 11;   // warp_row_tma: rows per CTA (+1 prod
 constexpr int64_t kWarpRowTmaMinL = 1024; // below two warp tiles the plain warp_row is as good
 constexpr int64_t kChunkedMinL = 8192;    // chunked (look-back) schedule: at least ~10 tiles per row
 constexpr int kSelWarps = 4;        // warp_row: rows per CTA
-constexpr int kLaneRowTc = 32;      // lane_row: timesteps per staged B/C tile
+#ifndef LR_TC
+#define LR_TC 32
+#endif
+constexpr int kLaneRowTc = LR_TC;   // lane_row: timesteps per staged B/C tile
 constexpr int kLaneRowWarps = 4;    // lane_row: warps per CTA (autonomous)
 constexpr int kLaneRowDefaultPoly16 = 4;  // sixteenths of the exps done on the fma pipe
 

@@ -12,15 +12,16 @@
 //     u    = {delta*x,delta*x} * Bpair       FMUL2
 //     h    = a*h + u                         FFMA2   (Eq.3 with the pair of P:86 Eq.6)
 //     y   += Cpair*h                         FFMA2   (BJ: y = sum_n C h + D x; h never stored)
-// issued "pass-major": one pass = four states over the VEC timesteps of a 128-bit group, first
-// every 2^x of the pass, then the dependent h chains.
-// A warp covers 32/G consecutive d of one batch b, so B_t/C_t are warp-uniform: each warp stages
-// its [2][N][TC] B/C tile with two TMA tensor copies per tile (cp.async.bulk.tensor.2d through
-// tensor maps over [batch*N, L], mbarrier complete_tx, double-buffered; SASS UTMALDG),
-// transposes/widens it once to an fp32 [TC][2][N] tile, and every state-step then reads B/C with
-// broadcast LDS.128.  x/delta come from global memory as raw 128-bit words prefetched two groups
-// ahead; y is reduced across the G lanes of the row with a shuffle reduce-scatter and leaves
-// with 128/G-bit stores.  Warps are autonomous: no CTA barrier.
+// issued "pass-major" for G = 1 (one pass = four states over the VEC timesteps of a 128-bit group,
+// first every 2^x of the pass, then the dependent h chains) and timestep-major for G >= 2.
+// A warp covers 32/G consecutive d of one batch b, so B_t/C_t are warp-uniform and are read from an
+// fp32 [TC][2][N] shared-memory tile with broadcast LDS.128.  The tile is staged either by the warp
+// itself (uniform grid: two TMA tensor copies per tile, cp.async.bulk.tensor.2d through tensor maps
+// over [batch*N, L], mbarrier complete_tx, double-buffered, SASS UTMALDG; then widened/transposed by
+// the warp) or once per CTA by a producer warp (balanced grid, selective_scan_lane_mix_kernel at
+// the end of this file).  x/delta come from global memory as raw 128-bit words prefetched PD groups
+// ahead; y is reduced across the G lanes of the row with a shuffle reduce-scatter and leaves with
+// 128/G-bit stores.  Row warps never meet at a CTA barrier.
 //
 // Template options:
 //   EXT   the fused steps either side of the scan, a bit mask: kExtSoftplus =
@@ -50,6 +51,16 @@ constexpr int kExtGeneric = kExtSoftplus | kExtGate | kExtReset | kExtRuntime;  
 __host__ __device__ constexpr bool lane_row_slot_is_poly(int idx, int F16)
 {
     return ((idx + 1) * F16) / 16 != (idx * F16) / 16;
+}
+
+// compile-time loop: f(integral_constant<int, I>) for I in [0, N)
+template <int I, int N, typename F>
+__device__ __forceinline__ void static_for(F&& f)
+{
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
 }
 
 // ------------------------------------------------------------------ shared-memory plan
@@ -142,7 +153,13 @@ struct RowSeg<__nv_bfloat16, 2> {
 // CTA-shared B/C tiles (lane_mix kernel): a producer warp stages the fp32 [TC][2][N] tiles of the
 // batches the CTA touches into a ring of kStages slots; consumers wait on full[slot] and arrive
 // on empty[slot] once per tile.
-constexpr int kMixStages = 3;
+#ifndef LR_PD
+#define LR_PD 2
+#endif
+#ifndef LR_MIX_STAGES
+#define LR_MIX_STAGES 4
+#endif
+constexpr int kMixStages = LR_MIX_STAGES;
 constexpr int kMixMaxBatches = 2;
 struct SharedTiles {
     const float* bc;   // [kMixStages][kMixMaxBatches][TC][2][N]
@@ -174,7 +191,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
     constexpr int YC = VEC / G;        // y values per lane after the reduce-scatter
     static_assert(G == 1 || G == 2 || G == 4, "G");
     static_assert(NP % PP == 0, "pairs per pass");
-    static_assert(NS % 4 == 0 && YC >= 1 && TC % VEC == 0 && (TC / VEC) % 2 == 0, "shape");
+    static_assert(NS % 4 == 0 && YC >= 1 && TC % VEC == 0 && (TC / VEC) % LR_PD == 0, "shape");
     static_assert(ASTR == 0 || (G == 1 && F16 == 0), "structured-A paths: one lane per row, no polynomial");
 
     const int lane = threadIdx.x & 31;
@@ -250,7 +267,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
     if (G >= 4) yoff += (g & 1) ? VEC / 4 : 0;
 
     // A1: raw 128-bit prefetch, two groups (2*VEC timesteps) ahead
-    constexpr int PD = 2;
+    constexpr int PD = LR_PD;  // 128-bit x/delta groups in flight per row
     uint4 xq[PD], dq[PD];
 #pragma unroll
     for (int i = 0; i < PD; ++i) {
@@ -294,225 +311,226 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
         // A3..A9: sequential in t.  One group = VEC timesteps of the warp's rows.
         auto group = [&](auto pitag, const int grp, const long long tg) {
             constexpr int PI = decltype(pitag)::value;
-                    float xv[VEC], dl[VEC];
-                    unpack128<T>(xq[PI], xv);
-                    unpack128<T>(dq[PI], dl);
-                    {   // refill the prefetch slot.  G >= 2 (four warps per sub-partition): always,
-                        // past the end of the row this group is re-read and never used (a
-                        // conditional refill costs a register copy per word: +2.5 %); G = 1:
-                        // conditional (measured: the unconditional form is scheduled late and
-                        // the one or two resident warps cannot hide it: 0.355 -> 0.425 ms)
-                        const long long tn = tg + PD * VEC;
-                        const long long ta = (G >= 2 && tn >= L) ? tg : tn;
-                        if (G >= 2 || tn < L) {
-                            xq[PI] = __ldcs(reinterpret_cast<const uint4*>(xr + ta));
-                            dq[PI] = __ldcs(reinterpret_cast<const uint4*>(dr + ta));
+            float xv[VEC], dl[VEC];
+            unpack128<T>(xq[PI], xv);
+            unpack128<T>(dq[PI], dl);
+            {   // refill the prefetch slot.  G >= 2 (four warps per sub-partition): always,
+                // past the end of the row this group is re-read and never used (a
+                // conditional refill costs a register copy per word: +2.5 %); G = 1:
+                // conditional (measured: the unconditional form is scheduled late and
+                // the one or two resident warps cannot hide it: 0.355 -> 0.425 ms)
+                const long long tn = tg + PD * VEC;
+                const long long ta = (G >= 2 && tn >= L) ? tg : tn;
+                if (G >= 2 || tn < L) {
+                    xq[PI] = __ldcs(reinterpret_cast<const uint4*>(xr + ta));
+                    dq[PI] = __ldcs(reinterpret_cast<const uint4*>(dr + ta));
+                }
+            }
+            // f1 prologue: Delta = softplus(delta + bias[d]); f2: reset bits of the group
+            unsigned rmask = 0;
+            float zv[YC];
+            if (EXT & kExtSoftplus) {
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    dl[k] += bias;
+                    if (!kRt || ext.delta_softplus) dl[k] = softplus_f(dl[k]);
+                }
+            }
+            if ((EXT & kExtReset) && rst) {
+#pragma unroll
+                for (int k = 0; k < VEC; ++k)
+                    rmask |= (__ldg(rst + tg + k) != 0 ? 1u : 0u) << k;
+            }
+            if ((EXT & kExtGate) && (!kRt || zr)) RowSeg<T, YC>::load(zr + tg + yoff, zv);
+            float ys[VEC];
+            float dxs[VEC];
+            pair_t y2[VEC];
+#pragma unroll
+            for (int k = 0; k < VEC; ++k) {
+                dxs[k] = dl[k] * xv[k];
+                y2[k] = pk(Dg * xv[k], 0.0f);
+            }
+            // structured A: the decay base r_k = 2^(delta_k A2[d,0]) of each timestep
+            pair_t cur[ASTR == 2 ? VEC : 1];
+            float r1[ASTR != 0 ? VEC : 1], r2[ASTR == 2 ? VEC : 1];
+            if (ASTR != 0) {
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    r1[k] = ex2_approx(dl[k] * A20);
+                    if (ASTR == 2) {
+                        r2[k] = r1[k] * r1[k];
+                        cur[k] = pk(r1[k], r2[k]);  // {r^1, r^2}; next pairs: * {r^2, r^2}
+                    }
+                }
+            }
+            // One pass = four states (two packed pairs, one LDS.128 of B and of C per
+            // timestep) over the VEC timesteps of the group: first every 2^x of the pass
+            // (independent: they stream through the MUFU / fma pipes back to back), then
+            // the two dependent h chains.  F = sixteenths of the exps taken by the
+            // polynomial (0 on the guarded slow path); RST = the group holds a reset.
+            auto pass = [&](int q, auto ftag, auto rtag) {
+                constexpr int F = decltype(ftag)::value;
+                constexpr bool RST = decltype(rtag)::value;
+                pair_t av[VEC][PP];
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) {
+                    const pair_t dd = pk(dl[k], dl[k]);
+#pragma unroll
+                    for (int s = 0; s < PP; ++s) {
+                        const int p = PP * q + s;
+                        if (ASTR == 1) {
+                            av[k][s] = pk(r1[k], r1[k]);
+                        } else if (ASTR == 2) {
+                            if (p > 0) cur[k] = mul2(cur[k], pk(r2[k], r2[k]));
+                            av[k][s] = cur[k];
+                        } else if (lane_row_slot_is_poly(k * NP + p, F)) {
+                            av[k][s] = exp2_poly2<DEG>(dd, A2p[p]);
+                        } else {
+                            float lo, hi;
+                            upk(mul2(dd, A2p[p]), lo, hi);
+                            av[k][s] = pk(ex2_approx(lo), ex2_approx(hi));
                         }
+                        // a reset step is the left-zero pair (0, u_t): h_{t-1} is dropped
+                        if (RST && ((rmask >> k) & 1u)) av[k][s] = pk(0.0f, 0.0f);
                     }
-                    // f1 prologue: Delta = softplus(delta + bias[d]); f2: reset bits of the group
-                    unsigned rmask = 0;
-                    float zv[YC];
-                    if (EXT & kExtSoftplus) {
+                }
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            dl[k] += bias;
-                            if (!kRt || ext.delta_softplus) dl[k] = softplus_f(dl[k]);
-                        }
+                for (int k = 0; k < VEC; ++k) {
+                    const pair_t dxx = pk(dxs[k], dxs[k]);
+                    const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 2 * PP * q;
+#pragma unroll
+                    for (int s = 0; s < PP; s += 2) {
+                        const int p = PP * q + s;
+                        const ulonglong2 b4 =
+                            *reinterpret_cast<const ulonglong2*>(bct + 2 * s);
+                        const ulonglong2 c4 =
+                            *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
+                        h2[p] = fma2(av[k][s], h2[p], mul2(dxx, b4.x));
+                        h2[p + 1] = fma2(av[k][s + 1], h2[p + 1], mul2(dxx, b4.y));
+                        y2[k] = fma2(c4.x, h2[p], y2[k]);
+                        y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
                     }
-                    if ((EXT & kExtReset) && rst) {
+                }
+            };
+            // ORDER == 1: timestep-major.  All the states of a lane for one timestep, then
+            // the next timestep: the MUFU, fma-pipe and LDS instructions of a warp come
+            // evenly mixed instead of in bursts (a burst of 2^x fills the SMSP's shared
+            // MIO queue and stalls the other warps' LDS: measured with 4 warps per SMSP).
+            auto steps = [&](auto ftag, auto rtag) {
+                constexpr int F = decltype(ftag)::value;
+                constexpr bool RST = decltype(rtag)::value;
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k)
-                            rmask |= (__ldg(rst + tg + k) != 0 ? 1u : 0u) << k;
-                    }
-                    if ((EXT & kExtGate) && (!kRt || zr)) RowSeg<T, YC>::load(zr + tg + yoff, zv);
-                    float ys[VEC];
-                    float dxs[VEC];
-                    pair_t y2[VEC];
+                for (int k = 0; k < VEC; ++k) {
+                    const pair_t dd = pk(dl[k], dl[k]);
+                    const pair_t dxx = pk(dxs[k], dxs[k]);
+                    const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS;
+                    const bool rs = RST && ((rmask >> k) & 1u);
 #pragma unroll
-                    for (int k = 0; k < VEC; ++k) {
-                        dxs[k] = dl[k] * xv[k];
-                        y2[k] = pk(Dg * xv[k], 0.0f);
-                    }
-                    // structured A: the decay base r_k = 2^(delta_k A2[d,0]) of each timestep
-                    pair_t cur[ASTR == 2 ? VEC : 1];
-                    float r1[ASTR != 0 ? VEC : 1], r2[ASTR == 2 ? VEC : 1];
-                    if (ASTR != 0) {
+                    for (int p = 0; p < NP; p += 2) {
+                        const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 2 * p);
+                        const ulonglong2 c4 =
+                            *reinterpret_cast<const ulonglong2*>(bct + N + 2 * p);
+                        pair_t a2[2];
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            r1[k] = ex2_approx(dl[k] * A20);
-                            if (ASTR == 2) {
-                                r2[k] = r1[k] * r1[k];
-                                cur[k] = pk(r1[k], r2[k]);  // {r^1, r^2}; next pairs: * {r^2, r^2}
+                        for (int s = 0; s < 2; ++s) {
+                            if (ASTR == 1) {
+                                a2[s] = pk(r1[k], r1[k]);
+                            } else if (ASTR == 2) {
+                                if (p + s > 0) cur[k] = mul2(cur[k], pk(r2[k], r2[k]));
+                                a2[s] = cur[k];
+                            } else if (lane_row_slot_is_poly(k * NP + p + s, F)) {
+                                a2[s] = exp2_poly2<DEG>(dd, A2p[p + s]);
+                            } else {
+                                float lo, hi;
+                                upk(mul2(dd, A2p[p + s]), lo, hi);
+                                a2[s] = pk(ex2_approx(lo), ex2_approx(hi));
                             }
+                            if (rs) a2[s] = pk(0.0f, 0.0f);
                         }
+                        h2[p] = fma2(a2[0], h2[p], mul2(dxx, b4.x));
+                        h2[p + 1] = fma2(a2[1], h2[p + 1], mul2(dxx, b4.y));
+                        y2[k] = fma2(c4.x, h2[p], y2[k]);
+                        y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
                     }
-                    // One pass = four states (two packed pairs, one LDS.128 of B and of C per
-                    // timestep) over the VEC timesteps of the group: first every 2^x of the pass
-                    // (independent: they stream through the MUFU / fma pipes back to back), then
-                    // the two dependent h chains.  F = sixteenths of the exps taken by the
-                    // polynomial (0 on the guarded slow path); RST = the group holds a reset.
-                    auto pass = [&](int q, auto ftag, auto rtag) {
-                        constexpr int F = decltype(ftag)::value;
-                        constexpr bool RST = decltype(rtag)::value;
-                        pair_t av[VEC][PP];
+                }
+            };
+            // the polynomial needs |delta*A2| <= 126; a group in which any lane of the
+            // warp exceeds that (a underflows: far outside BJ's distributions) takes the
+            // all-MUFU path instead, so nothing is ever clamped
+            bool poly_ok = true;
+            if (F16 > 0) {
+                float dm = fabsf(dl[0]);
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            const pair_t dd = pk(dl[k], dl[k]);
+                for (int k = 1; k < VEC; ++k) dm = fmaxf(dm, fabsf(dl[k]));
+                poly_ok = !__any_sync(kFullMask, !(dm <= dmax));
+            }
+            if (ORDER == 1) {
+                if ((EXT & kExtReset) && rmask != 0)
+                    steps(std::integral_constant<int, 0>{}, std::true_type{});
+                else if (poly_ok) steps(std::integral_constant<int, F16>{}, std::false_type{});
+                else steps(std::integral_constant<int, 0>{}, std::false_type{});
+            } else if ((EXT & kExtReset) && rmask != 0) {  // warp-uniform (rows of a warp share b)
 #pragma unroll
-                            for (int s = 0; s < PP; ++s) {
-                                const int p = PP * q + s;
-                                if (ASTR == 1) {
-                                    av[k][s] = pk(r1[k], r1[k]);
-                                } else if (ASTR == 2) {
-                                    if (p > 0) cur[k] = mul2(cur[k], pk(r2[k], r2[k]));
-                                    av[k][s] = cur[k];
-                                } else if (lane_row_slot_is_poly(k * NP + p, F)) {
-                                    av[k][s] = exp2_poly2<DEG>(dd, A2p[p]);
-                                } else {
-                                    float lo, hi;
-                                    upk(mul2(dd, A2p[p]), lo, hi);
-                                    av[k][s] = pk(ex2_approx(lo), ex2_approx(hi));
-                                }
-                                // a reset step is the left-zero pair (0, u_t): h_{t-1} is dropped
-                                if (RST && ((rmask >> k) & 1u)) av[k][s] = pk(0.0f, 0.0f);
-                            }
-                        }
+                for (int q = 0; q < NP / PP; ++q)
+                    pass(q, std::integral_constant<int, 0>{}, std::true_type{});
+            } else if (poly_ok) {
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            const pair_t dxx = pk(dxs[k], dxs[k]);
-                            const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS + 2 * PP * q;
+                for (int q = 0; q < NP / PP; ++q)
+                    pass(q, std::integral_constant<int, F16>{}, std::false_type{});
+            } else {
 #pragma unroll
-                            for (int s = 0; s < PP; s += 2) {
-                                const int p = PP * q + s;
-                                const ulonglong2 b4 =
-                                    *reinterpret_cast<const ulonglong2*>(bct + 2 * s);
-                                const ulonglong2 c4 =
-                                    *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
-                                h2[p] = fma2(av[k][s], h2[p], mul2(dxx, b4.x));
-                                h2[p + 1] = fma2(av[k][s + 1], h2[p + 1], mul2(dxx, b4.y));
-                                y2[k] = fma2(c4.x, h2[p], y2[k]);
-                                y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
-                            }
-                        }
-                    };
-                    // ORDER == 1: timestep-major.  All the states of a lane for one timestep, then
-                    // the next timestep: the MUFU, fma-pipe and LDS instructions of a warp come
-                    // evenly mixed instead of in bursts (a burst of 2^x fills the SMSP's shared
-                    // MIO queue and stalls the other warps' LDS: measured with 4 warps per SMSP).
-                    auto steps = [&](auto ftag, auto rtag) {
-                        constexpr int F = decltype(ftag)::value;
-                        constexpr bool RST = decltype(rtag)::value;
+                for (int q = 0; q < NP / PP; ++q)
+                    pass(q, std::integral_constant<int, 0>{}, std::false_type{});
+            }
 #pragma unroll
-                        for (int k = 0; k < VEC; ++k) {
-                            const pair_t dd = pk(dl[k], dl[k]);
-                            const pair_t dxx = pk(dxs[k], dxs[k]);
-                            const float* bct = bc + (grp * VEC + k) * 2 * N + g * NS;
-                            const bool rs = RST && ((rmask >> k) & 1u);
+            for (int k = 0; k < VEC; ++k) {
+                float ylo, yhi;
+                upk(y2[k], ylo, yhi);
+                ys[k] = ylo + yhi;
+            }
+            // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
+            // each lane ends with YC fully reduced timesteps) and store
+            if (G >= 2) {
+                const bool up = (g & (G / 2)) != 0;
 #pragma unroll
-                            for (int p = 0; p < NP; p += 2) {
-                                const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 2 * p);
-                                const ulonglong2 c4 =
-                                    *reinterpret_cast<const ulonglong2*>(bct + N + 2 * p);
-                                pair_t a2[2];
+                for (int j = 0; j < VEC / 2; ++j) {
+                    const float mine = up ? ys[VEC / 2 + j] : ys[j];
+                    const float send = up ? ys[j] : ys[VEC / 2 + j];
+                    ys[j] = mine + __shfl_xor_sync(kFullMask, send, G / 2);
+                }
+            }
+            if (G >= 4) {
+                const bool up = (g & 1) != 0;
 #pragma unroll
-                                for (int s = 0; s < 2; ++s) {
-                                    if (ASTR == 1) {
-                                        a2[s] = pk(r1[k], r1[k]);
-                                    } else if (ASTR == 2) {
-                                        if (p + s > 0) cur[k] = mul2(cur[k], pk(r2[k], r2[k]));
-                                        a2[s] = cur[k];
-                                    } else if (lane_row_slot_is_poly(k * NP + p + s, F)) {
-                                        a2[s] = exp2_poly2<DEG>(dd, A2p[p + s]);
-                                    } else {
-                                        float lo, hi;
-                                        upk(mul2(dd, A2p[p + s]), lo, hi);
-                                        a2[s] = pk(ex2_approx(lo), ex2_approx(hi));
-                                    }
-                                    if (rs) a2[s] = pk(0.0f, 0.0f);
-                                }
-                                h2[p] = fma2(a2[0], h2[p], mul2(dxx, b4.x));
-                                h2[p + 1] = fma2(a2[1], h2[p + 1], mul2(dxx, b4.y));
-                                y2[k] = fma2(c4.x, h2[p], y2[k]);
-                                y2[k] = fma2(c4.y, h2[p + 1], y2[k]);
-                            }
-                        }
-                    };
-                    // the polynomial needs |delta*A2| <= 126; a group in which any lane of the
-                    // warp exceeds that (a underflows: far outside BJ's distributions) takes the
-                    // all-MUFU path instead, so nothing is ever clamped
-                    bool poly_ok = true;
-                    if (F16 > 0) {
-                        float dm = fabsf(dl[0]);
+                for (int j = 0; j < VEC / 4; ++j) {
+                    const float mine = up ? ys[VEC / 4 + j] : ys[j];
+                    const float send = up ? ys[j] : ys[VEC / 4 + j];
+                    ys[j] = mine + __shfl_xor_sync(kFullMask, send, 1);
+                }
+            }
+            float out[YC];
 #pragma unroll
-                        for (int k = 1; k < VEC; ++k) dm = fmaxf(dm, fabsf(dl[k]));
-                        poly_ok = !__any_sync(kFullMask, !(dm <= dmax));
-                    }
-                    if (ORDER == 1) {
-                        if ((EXT & kExtReset) && rmask != 0)
-                            steps(std::integral_constant<int, 0>{}, std::true_type{});
-                        else if (poly_ok) steps(std::integral_constant<int, F16>{}, std::false_type{});
-                        else steps(std::integral_constant<int, 0>{}, std::false_type{});
-                    } else if ((EXT & kExtReset) && rmask != 0) {  // warp-uniform (rows of a warp share b)
+            for (int j = 0; j < YC; ++j) out[j] = ys[j];
+            if ((EXT & kExtGate) && (!kRt || zr)) {  // f1 epilogue: y <- y * silu(z)
 #pragma unroll
-                        for (int q = 0; q < NP / PP; ++q)
-                            pass(q, std::integral_constant<int, 0>{}, std::true_type{});
-                    } else if (poly_ok) {
-#pragma unroll
-                        for (int q = 0; q < NP / PP; ++q)
-                            pass(q, std::integral_constant<int, F16>{}, std::false_type{});
-                    } else {
-#pragma unroll
-                        for (int q = 0; q < NP / PP; ++q)
-                            pass(q, std::integral_constant<int, 0>{}, std::false_type{});
-                    }
-#pragma unroll
-                    for (int k = 0; k < VEC; ++k) {
-                        float ylo, yhi;
-                        upk(y2[k], ylo, yhi);
-                        ys[k] = ylo + yhi;
-                    }
-                    // A9: reduce the partial sums over the G lanes of the row (reduce-scatter:
-                    // each lane ends with YC fully reduced timesteps) and store
-                    if (G >= 2) {
-                        const bool up = (g & (G / 2)) != 0;
-#pragma unroll
-                        for (int j = 0; j < VEC / 2; ++j) {
-                            const float mine = up ? ys[VEC / 2 + j] : ys[j];
-                            const float send = up ? ys[j] : ys[VEC / 2 + j];
-                            ys[j] = mine + __shfl_xor_sync(kFullMask, send, G / 2);
-                        }
-                    }
-                    if (G >= 4) {
-                        const bool up = (g & 1) != 0;
-#pragma unroll
-                        for (int j = 0; j < VEC / 4; ++j) {
-                            const float mine = up ? ys[VEC / 4 + j] : ys[j];
-                            const float send = up ? ys[j] : ys[VEC / 4 + j];
-                            ys[j] = mine + __shfl_xor_sync(kFullMask, send, 1);
-                        }
-                    }
-                    float out[YC];
-#pragma unroll
-                    for (int j = 0; j < YC; ++j) out[j] = ys[j];
-                    if ((EXT & kExtGate) && (!kRt || zr)) {  // f1 epilogue: y <- y * silu(z)
-#pragma unroll
-                        for (int j = 0; j < YC; ++j) out[j] *= silu_io<T>(zv[j]);
-                    }
-                    if (y) RowSeg<T, YC>::store(yr + tg + yoff, out);  // y == NULL: aggregate-only call
+                for (int j = 0; j < YC; ++j) out[j] *= silu_io<T>(zv[j]);
+            }
+            if (y) RowSeg<T, YC>::store(yr + tg + yoff, out);  // y == NULL: aggregate-only call
         };
         if (G >= 2 && t0 + TC <= L) {  // whole tile inside the row: no per-group conditions
 #pragma unroll 1
-            for (int gi = 0; gi < kChunks; gi += PD) {
-                group(std::integral_constant<int, 0>{}, gi, t0 + gi * VEC);
-                group(std::integral_constant<int, 1>{}, gi + 1, t0 + (gi + 1) * VEC);
-            }
+            for (int gi = 0; gi < kChunks; gi += PD)
+                static_for<0, PD>([&](auto pi) {
+                    constexpr int PI = decltype(pi)::value;
+                    group(pi, gi + PI, t0 + (gi + PI) * VEC);
+                });
         } else {
 #pragma unroll 1
-            for (int gi = 0; gi < kChunks; gi += PD) {
-                if (t0 + gi * VEC < L) group(std::integral_constant<int, 0>{}, gi, t0 + gi * VEC);
-                if (t0 + (gi + 1) * VEC < L)
-                    group(std::integral_constant<int, 1>{}, gi + 1, t0 + (gi + 1) * VEC);
-            }
+            for (int gi = 0; gi < kChunks; gi += PD)
+                static_for<0, PD>([&](auto pi) {
+                    constexpr int PI = decltype(pi)::value;
+                    if (t0 + (gi + PI) * VEC < L) group(pi, gi + PI, t0 + (gi + PI) * VEC);
+                });
         }
         if (SHARED) {  // this warp is done with the slot
             __syncwarp();

@@ -328,7 +328,8 @@ AFFINESCAN_API int affinescan_version(void);
 typedef enum affinescan_option {
     AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lane_row grid: 1 or 2 lanes per (b,d) row; 3 = balanced mix */
     AFFINESCAN_OPT_LANE_ROW_POLY16 = 2  /* sixteenths (0 or 4) of the exponentials evaluated by
-                                           the fma-pipe polynomial instead of MUFU.EX2           */
+                                           the fma-pipe polynomial instead of MUFU.EX2 (one-lane
+                                           grid only; the other grids ignore it)                 */
 } affinescan_option;
 AFFINESCAN_API int affinescan_set_option(int key, int value);
 /* Frees the cached scratch / staging buffers, copy streams and events of the current device

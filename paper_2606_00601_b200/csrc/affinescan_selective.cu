@@ -263,8 +263,9 @@ int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
     }
     if (G == 1 && poly16 == 0) return launch_lane_row_gf<T, 1, 0>(t, stream);
     if (G == 1 && poly16 == 4) return launch_lane_row_gf<T, 1, 4>(t, stream);
-    if (G == 2 && poly16 == 0) return launch_lane_row_gf<T, 2, 0>(t, stream);
-    if (G == 2 && poly16 == 4) return launch_lane_row_gf<T, 2, 4>(t, stream);
+    // the polynomial only pays with one or two warps per sub-partition: the
+    // two-lane and balanced grids always take every 2^x on the MUFU
+    if (G == 2) return launch_lane_row_gf<T, 2, 0>(t, stream);
     return AFFINESCAN_ERR_UNSUPPORTED;
 }
 

@@ -288,7 +288,7 @@ AFFINESCAN_API int affinescan_compose_carry(const float* P_all, const float* U_a
  * h_t = a_t h_{t-1} + u_t (Eq.3) is the same affine recurrence run right to left,
  * g_t = a_{t+1} g_{t+1} + C_t dy_t, i.e. the scan of P:90 Eq.(7) over the reversed sequence;
  * h_{t-1} is recomputed from checkpoints kept in library scratch (8 B per (b,d,t) for the
- * checkpoints + 4 B for the dB/dC partial sums, stream-ordered), never divided out.
+ * checkpoints + 8 B for the dB/dC partial sums, stream-ordered), never divided out.
  *
  *   x, delta, dy [batch, d_inner, L] io dtype  in      A [d_inner, N] fp32   in
  *   B, C         [batch, N, L]       io dtype  in      D [d_inner]    fp32   in, NULL => 0
@@ -299,7 +299,8 @@ AFFINESCAN_API int affinescan_compose_carry(const float* P_all, const float* U_a
  *   dh0          [batch, d_inner, N] fp32      out
  * Every output pointer may be NULL (=> not written).  All gradients are fp32 whatever the io
  * dtype; sums over rows and batches are formed in a fixed order (bitwise reproducible).
- * Supported shapes: N == 16, d_inner % 32 == 0, L % 8 == 0, 16-byte aligned pointers; anything
+ * Supported shapes: N == 16, d_inner % 32 == 0, L % 8 == 0, 16-byte aligned pointers (dx and
+ * ddelta included); anything
  * else returns AFFINESCAN_ERR_UNSUPPORTED.  Asynchronous on cuda_stream.
  * ------------------------------------------------------------------------------------ */
 AFFINESCAN_API int selective_scan_bwd(const void* x, const void* delta, const float* A,

@@ -39,10 +39,10 @@ template <typename T>
 int bwd_launch(const BwdArgs& a, cudaStream_t stream)
 {
     const int64_t rows = static_cast<int64_t>(a.batch) * a.d_inner;
-    const int64_t groups = rows / 32;
+    const int64_t groups = rows / kBwdRW;
     const int64_t nchunks = a.L / kBwdCK;
     // scratch: [ckpt | part | dA_part | dD_part], all fp32
-    const size_t n_ckpt = static_cast<size_t>(groups) * nchunks * kBwdN * 32;
+    const size_t n_ckpt = static_cast<size_t>(groups) * nchunks * kBwdN * kBwdRW;
     const size_t n_part = static_cast<size_t>(groups) * a.L * 2 * kBwdN;
     const size_t n_da = static_cast<size_t>(rows) * kBwdN;
     const size_t n_dd = static_cast<size_t>(rows);
@@ -72,7 +72,7 @@ int bwd_launch(const BwdArgs& a, cudaStream_t stream)
     if (st == AFFINESCAN_OK && (a.dB || a.dC)) {
         const dim3 grid(static_cast<unsigned>((a.L + 31) / 32), static_cast<unsigned>(a.batch));
         selective_scan_bwd_reduce_bc_kernel<<<grid, 1024, 0, stream>>>(part, a.dB, a.dC,
-                                                                       a.d_inner / 32, a.L);
+                                                                       a.d_inner / kBwdRW, a.L);
         st = after_launch();
     }
     if (st == AFFINESCAN_OK && (a.dA || a.dD)) {
@@ -114,10 +114,11 @@ extern "C" int selective_scan_bwd(const void* x, const void* delta, const float*
         return copy_or_zero(dh_last, dh0, rows * N, stream);
     }
     if (!x || !delta || !A || !B || !C || !dy) return AFFINESCAN_ERR_NULL;
-    // the tuned layout only: N = 16, one lane per row with 32 rows of one batch per warp,
-    // 128-bit loads along L, 8-step checkpoint chunks
+    // the tuned layout only: N = 16, two lanes per row with 16 rows of one batch per warp,
+    // 128-bit accesses along L, 8-step checkpoint chunks
     if (N != kBwdN || d_inner % 32 != 0 || L % kBwdCK != 0 || !aligned16(x) || !aligned16(delta) ||
-        !aligned16(B) || !aligned16(C) || !aligned16(dy) || !aligned16(A))
+        !aligned16(B) || !aligned16(C) || !aligned16(dy) || !aligned16(A) || !aligned16(dx) ||
+        !aligned16(ddelta))
         return AFFINESCAN_ERR_UNSUPPORTED;
     const BwdArgs a{x, delta, B, C, dy, A, D, h0, dh_last, dx, ddelta, dA, dB, dC, dD, dh0,
                     batch, d_inner, N, L};

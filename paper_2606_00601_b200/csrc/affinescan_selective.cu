@@ -206,7 +206,7 @@ int launch_lane_mix_inst(const Typed<T>& t, cudaStream_t stream)
     AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
     int sms = 0;
     AS_TRY(sm_count(&sms));
-    kern<<<static_cast<unsigned>(sms), 17 * 32, smem, stream>>>(
+    kern<<<static_cast<unsigned>(sms), 16 * 32, smem, stream>>>(
         t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner, t.L);
     return after_launch();
 }

@@ -168,6 +168,73 @@ struct SharedTiles {
     int bsel;          // which of the CTA's batches this warp's rows belong to
 };
 
+// The staging duty of the balanced grid: TMA tensor copies of the raw [2N][TC] boxes of the CTA's
+// batches into a two-slot raw ring, widened and transposed (lane j = raw row j) into the ring of
+// fp32 tiles.  Run by ONE warp of the CTA — a row warp that stages tile i + kMixStages - 1 before
+// it consumes tile i, or on its own when that warp has no rows.
+template <typename T, int TC>
+struct MixStager {
+    using S = LaneRowSmem<T, TC>;
+    const CUtensorMap* mapB;
+    const CUtensorMap* mapC;
+    float* bc_ring;
+    unsigned char* raw_ring;
+    uint64_t* full;
+    uint64_t* empty;
+    uint64_t* raw_full;
+    int b_first, nb;
+    long long ntiles;
+
+    __device__ __forceinline__ void issue_raw(long long tile, int lane) const
+    {
+        if (lane == 0) {
+            const int rs = static_cast<int>(tile & 1);
+            const int t0 = static_cast<int>(tile * TC);
+            mbar_arrive_expect_tx(&raw_full[rs], static_cast<unsigned>(nb * S::kRawStage));
+            for (int j = 0; j < nb; ++j) {
+                unsigned char* dst = raw_ring + (rs * kMixMaxBatches + j) * S::kRawStage;
+                tma_tile_2d_g2s(dst, mapB, t0, (b_first + j) * S::N, &raw_full[rs]);
+                tma_tile_2d_g2s(dst + S::N * S::kRawPitch, mapC, t0, (b_first + j) * S::N,
+                                &raw_full[rs]);
+            }
+        }
+    }
+    __device__ __forceinline__ void stage(long long tile, int lane) const
+    {
+        constexpr int VEC = Io<T>::kVec;
+        const int slot = static_cast<int>(tile % kMixStages);
+        const int rs = static_cast<int>(tile & 1);
+        if (tile >= kMixStages)  // every row warp is done with the tile that held this slot
+            mbar_wait(&empty[slot], static_cast<unsigned>((tile / kMixStages - 1) & 1));
+        mbar_wait(&raw_full[rs], static_cast<unsigned>((tile >> 1) & 1));
+        for (int j = 0; j < nb; ++j) {
+            const unsigned char* src =
+                raw_ring + (rs * kMixMaxBatches + j) * S::kRawStage + lane * S::kRawPitch;
+            float* dst = bc_ring + (slot * kMixMaxBatches + j) * (TC * 2 * S::N);
+#pragma unroll
+            for (int c = 0; c < TC / VEC; ++c) {
+                float v[VEC];
+                unpack128<T>(*reinterpret_cast<const uint4*>(src + c * 16), v);
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) dst[(c * VEC + k) * 2 * S::N + lane] = v[k];
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&full[slot]);
+        if (tile + 2 < ntiles) {
+            fence_proxy_async_smem();  // generic reads of the raw slot before the async overwrite
+            issue_raw(tile + 2, lane);
+        }
+    }
+    // tiles 0 .. kMixStages - 2 (no slot is in use yet)
+    __device__ __forceinline__ void prologue(int lane) const
+    {
+        issue_raw(0, lane);
+        if (ntiles > 1) issue_raw(1, lane);
+        for (long long t = 0; t < kMixStages - 1 && t < ntiles; ++t) stage(t, lane);
+    }
+};
+
 // The work of ONE warp: RW = 32/G consecutive rows starting at row0 (all in one batch), walked
 // over the whole of L.  SHARED == false: `wbase` is the warp's private
 // LaneRowSmem<T, TC>::kPerWarp bytes and the warp stages its own B/C tiles; SHARED == true: the
@@ -179,7 +246,8 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
               const CUtensorMap* mapB, const CUtensorMap* mapC, const float* __restrict__ D,
               const float* __restrict__ h0, T* __restrict__ y, float* __restrict__ h_last,
               const SelectiveExt& ext, int d_inner, long long L, long long row0,
-              unsigned char* wbase, const SharedTiles sh = SharedTiles{})
+              unsigned char* wbase, const SharedTiles sh = SharedTiles{},
+              const MixStager<T, TC>* stg = nullptr)
 {
     using S = LaneRowSmem<T, TC>;
     constexpr int N = S::N;
@@ -279,10 +347,12 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
         }
     }
 
+    if (SHARED && stg) stg->prologue(lane);
     for (long long tile = 0; tile < ntiles; ++tile) {
         const long long t0 = tile * TC;
         int slot = 0;
         if (SHARED) {
+            if (stg && tile + kMixStages - 1 < ntiles) stg->stage(tile + kMixStages - 1, lane);
             slot = static_cast<int>(tile % kMixStages);
             mbar_wait(&full[slot], static_cast<unsigned>((tile / kMixStages) & 1));
             bc = sh.bc + (slot * kMixMaxBatches + sh.bsel) * (TC * 2 * N);
@@ -309,8 +379,12 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
         }
 
         // A3..A9: sequential in t.  One group = VEC timesteps of the warp's rows.
-        auto group = [&](auto pitag, const int grp, const long long tg) {
+        // `fasttag`: the group and its prefetch refill lie inside the row, so every address is the
+        // tile's base pointer plus a constant (no 64-bit position arithmetic per group)
+        auto group = [&](auto pitag, auto fasttag, const int grp, const long long tg, const T* xg,
+                         const T* dg, T* yg) {
             constexpr int PI = decltype(pitag)::value;
+            constexpr bool FAST = decltype(fasttag)::value;
             float xv[VEC], dl[VEC];
             unpack128<T>(xq[PI], xv);
             unpack128<T>(dq[PI], dl);
@@ -319,11 +393,16 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                 // conditional refill costs a register copy per word: +2.5 %); G = 1:
                 // conditional (measured: the unconditional form is scheduled late and
                 // the one or two resident warps cannot hide it: 0.355 -> 0.425 ms)
-                const long long tn = tg + PD * VEC;
-                const long long ta = (G >= 2 && tn >= L) ? tg : tn;
-                if (G >= 2 || tn < L) {
-                    xq[PI] = __ldcs(reinterpret_cast<const uint4*>(xr + ta));
-                    dq[PI] = __ldcs(reinterpret_cast<const uint4*>(dr + ta));
+                if (FAST) {
+                    xq[PI] = __ldcs(reinterpret_cast<const uint4*>(xg + PD * VEC));
+                    dq[PI] = __ldcs(reinterpret_cast<const uint4*>(dg + PD * VEC));
+                } else {
+                    const long long tn = tg + PD * VEC;
+                    const long long ta = (G >= 2 && tn >= L) ? tg : tn;
+                    if (G >= 2 || tn < L) {
+                        xq[PI] = __ldcs(reinterpret_cast<const uint4*>(xr + ta));
+                        dq[PI] = __ldcs(reinterpret_cast<const uint4*>(dr + ta));
+                    }
                 }
             }
             // f1 prologue: Delta = softplus(delta + bias[d]); f2: reset bits of the group
@@ -515,21 +594,30 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
 #pragma unroll
                 for (int j = 0; j < YC; ++j) out[j] *= silu_io<T>(zv[j]);
             }
-            if (y) RowSeg<T, YC>::store(yr + tg + yoff, out);  // y == NULL: aggregate-only call
+            if (y) RowSeg<T, YC>::store(yg, out);  // y == NULL: aggregate-only call
         };
-        if (G >= 2 && t0 + TC <= L) {  // whole tile inside the row: no per-group conditions
+        if (G >= 2 && t0 + TC + PD * VEC <= L) {  // tile and its prefetch inside the row
+            const T* xp = xr + t0;
+            const T* dp = dr + t0;
+            T* yp = yr + t0 + yoff;
 #pragma unroll 1
-            for (int gi = 0; gi < kChunks; gi += PD)
+            for (int gi = 0; gi < kChunks; gi += PD) {
                 static_for<0, PD>([&](auto pi) {
                     constexpr int PI = decltype(pi)::value;
-                    group(pi, gi + PI, t0 + (gi + PI) * VEC);
+                    group(pi, std::true_type{}, gi + PI, t0 + (gi + PI) * VEC, xp + PI * VEC,
+                          dp + PI * VEC, yp + PI * VEC);
                 });
+                xp += PD * VEC;
+                dp += PD * VEC;
+                yp += PD * VEC;
+            }
         } else {
 #pragma unroll 1
             for (int gi = 0; gi < kChunks; gi += PD)
                 static_for<0, PD>([&](auto pi) {
                     constexpr int PI = decltype(pi)::value;
-                    if (t0 + (gi + PI) * VEC < L) group(pi, gi + PI, t0 + (gi + PI) * VEC);
+                    const long long tg = t0 + (gi + PI) * VEC;
+                    if (tg < L) group(pi, std::false_type{}, gi + PI, tg, xr + tg, dr + tg, yr + tg + yoff);
                 });
         }
         if (SHARED) {  // this warp is done with the slot
@@ -574,15 +662,15 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 }
 
 // ====================================================================================
-// Balanced grid (one CTA per SM: 16 row warps + 1 producer warp): the XU pipe of a sub-partition
+// Balanced grid (one CTA of 16 row warps per SM): the XU pipe of a sub-partition
 // is the wall, and with R rows the uniform grid leaves sub-partitions holding ceil(...) warps
 // next to ones holding floor(...).  Here every sub-partition gets three G = 2 warps (16 rows
 // each) and one G = 4 warp (8 rows): 56 rows = 7/8 of what two G = 1 warps carry, spread over
 // four warps whose MUFU, fma and LDS instructions interleave.  Warp w of a CTA runs on
 // sub-partition w % 4.  CTA c owns rows [224 c, 224 c + 224) of a round (rounds of grid * 224
 // rows): the first 192 go to the G = 2 warps, the last 32 to the G = 4 warps.  Those rows lie in
-// at most kMixMaxBatches batches (the launcher checks d_inner), whose B/C tiles the producer
-// warp stages ONCE for the whole CTA: TMA tensor copies of the raw [2N][TC] boxes into a
+// at most kMixMaxBatches batches (the launcher checks d_inner), whose B/C tiles one of the
+// G = 4 warps (MixStager) stages ONCE for the whole CTA, kMixStages - 1 tiles ahead of its own row work: TMA tensor copies of the raw [2N][TC] boxes into a
 // two-slot raw ring, widened and transposed into a kMixStages-deep ring of fp32 [TC][2][N]
 // tiles that the row warps read with broadcast LDS.128.
 // ====================================================================================
@@ -596,7 +684,7 @@ struct LaneMixSmem {
 };
 
 template <typename T, int TC, int F16, int DEG, int EXT, int ORDER>
-__global__ void __launch_bounds__(17 * 32, 1)
+__global__ void __launch_bounds__(16 * 32, 1)
 selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ delta,
                                const float* __restrict__ A,
                                const __grid_constant__ CUtensorMap mapB,
@@ -607,11 +695,8 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
                                int d_inner, long long L)
 {
     using M = LaneMixSmem<T, TC>;
-    using S = LaneRowSmem<T, TC>;
-    constexpr int N = S::N;
-    constexpr int VEC = Io<T>::kVec;
-    constexpr int kChunks = TC / VEC;
     constexpr int kRowsPerCta = 12 * 16 + 4 * 8;
+    constexpr int kStagerWarp = 12;  // the first G = 4 warp also stages the CTA's B/C tiles
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* bc_ring = reinterpret_cast<float*>(smem_raw);
     unsigned char* raw_ring = smem_raw + M::kBcBytes;
@@ -653,67 +738,40 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
         fence_proxy_async_smem();
         __syncthreads();
 
-        if (warp == 16) {
-            // ------------------------------------------------------------ producer warp
-            auto issue_raw = [&](long long tile) {
-                if (lane == 0) {
-                    const int rs = static_cast<int>(tile & 1);
-                    const int t0 = static_cast<int>(tile * TC);
-                    mbar_arrive_expect_tx(&raw_full[rs], static_cast<unsigned>(nb * S::kRawStage));
-                    for (int j = 0; j < nb; ++j) {
-                        unsigned char* dst = raw_ring + (rs * kMixMaxBatches + j) * S::kRawStage;
-                        tma_tile_2d_g2s(dst, &mapB, t0, (b_first + j) * N, &raw_full[rs]);
-                        tma_tile_2d_g2s(dst + N * S::kRawPitch, &mapC, t0, (b_first + j) * N,
-                                        &raw_full[rs]);
-                    }
-                }
-            };
-            issue_raw(0);
-            if (ntiles > 1) issue_raw(1);
-            for (long long tile = 0; tile < ntiles; ++tile) {
-                const int slot = static_cast<int>(tile % kMixStages);
-                const int rs = static_cast<int>(tile & 1);
-                if (tile >= kMixStages)
-                    mbar_wait(&empty[slot], static_cast<unsigned>((tile / kMixStages - 1) & 1));
-                mbar_wait(&raw_full[rs], static_cast<unsigned>((tile >> 1) & 1));
-                for (int j = 0; j < nb; ++j) {
-                    const unsigned char* src =
-                        raw_ring + (rs * kMixMaxBatches + j) * S::kRawStage + lane * S::kRawPitch;
-                    float* dst = bc_ring + (slot * kMixMaxBatches + j) * (TC * 2 * N);
-#pragma unroll
-                    for (int c = 0; c < kChunks; ++c) {
-                        float v[VEC];
-                        unpack128<T>(*reinterpret_cast<const uint4*>(src + c * 16), v);
-#pragma unroll
-                        for (int k = 0; k < VEC; ++k) dst[(c * VEC + k) * 2 * N + lane] = v[k];
-                    }
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&full[slot]);
-                if (tile + 2 < ntiles) {
-                    fence_proxy_async_smem();  // generic reads of the raw slot before the async overwrite
-                    issue_raw(tile + 2);
-                }
-            }
-        } else {
-            // ------------------------------------------------------------ row warps
-            SharedTiles sh;
-            sh.bc = bc_ring;
-            sh.full = full;
-            sh.empty = empty;
-            if (warp < 12) {
-                if (warp < n2) {
-                    const long long row0 = cta0 + warp * 16;
-                    sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
-                    lane_row_warp<T, 2, TC, F16, DEG, EXT, 0, ORDER, true>(
-                        x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh);
-                }
-            } else if (warp - 12 < n4) {
-                const long long row0 = cta0 + r2 + (warp - 12) * 8;
+        MixStager<T, TC> stager;
+        stager.mapB = &mapB;
+        stager.mapC = &mapC;
+        stager.bc_ring = bc_ring;
+        stager.raw_ring = raw_ring;
+        stager.full = full;
+        stager.empty = empty;
+        stager.raw_full = raw_full;
+        stager.b_first = b_first;
+        stager.nb = nb;
+        stager.ntiles = ntiles;
+        SharedTiles sh;
+        sh.bc = bc_ring;
+        sh.full = full;
+        sh.empty = empty;
+        sh.bsel = 0;
+        if (warp < 12) {
+            if (warp < n2) {
+                const long long row0 = cta0 + warp * 16;
                 sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
-                lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true>(
+                lane_row_warp<T, 2, TC, F16, DEG, EXT, 0, ORDER, true>(
                     x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh);
             }
+        } else if (warp - 12 < n4) {
+            const long long row0 = cta0 + r2 + (warp - 12) * 8;
+            sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
+            lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true>(
+                x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh,
+                warp == kStagerWarp ? &stager : nullptr);
+        } else if (warp == kStagerWarp) {
+            // a last CTA without rows for this warp: staging only
+            stager.issue_raw(0, lane);
+            if (ntiles > 1) stager.issue_raw(1, lane);
+            for (long long tile = 0; tile < ntiles; ++tile) stager.stage(tile, lane);
         }
     }
 }

@@ -62,21 +62,23 @@ int get_encode_tiled(EncodeTiledFn* out)
 struct MapKey {
     const void* base;
     int64_t rows, L;
-    int box_t, N, esize;
+    int box_t, N, esize, swizzle;
     bool operator<(const MapKey& o) const
     {
-        return std::tie(base, rows, L, box_t, N, esize) <
-               std::tie(o.base, o.rows, o.L, o.box_t, o.N, o.esize);
+        return std::tie(base, rows, L, box_t, N, esize, swizzle) <
+               std::tie(o.base, o.rows, o.L, o.box_t, o.N, o.esize, o.swizzle);
     }
 };
 std::mutex g_map_mu;
 std::map<MapKey, CUtensorMap> g_maps;
 constexpr size_t kMaxCachedMaps = 512;
 
+// swizzle128 = the 128-byte shared-memory swizzle (box rows of exactly 128 B: the x / delta rings)
 template <typename T>
-int make_bc_tensor_map(CUtensorMap* map, const T* base, int64_t rows, int64_t L, int box_t, int N)
+int make_bc_tensor_map(CUtensorMap* map, const T* base, int64_t rows, int64_t L, int box_t, int N,
+                       bool swizzle128 = false)
 {
-    const MapKey key{base, rows, L, box_t, N, static_cast<int>(sizeof(T))};
+    const MapKey key{base, rows, L, box_t, N, static_cast<int>(sizeof(T)), swizzle128 ? 1 : 0};
     {
         std::lock_guard<std::mutex> lk(g_map_mu);
         auto it = g_maps.find(key);
@@ -94,7 +96,8 @@ int make_bc_tensor_map(CUtensorMap* map, const T* base, int64_t rows, int64_t L,
     const CUresult r = encode(map, sizeof(T) == 2 ? CU_TENSOR_MAP_DATA_TYPE_BFLOAT16
                                                   : CU_TENSOR_MAP_DATA_TYPE_FLOAT32,
                               2, const_cast<T*>(base), dims, strides, box, estr,
-                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) return cuda_fail(cudaErrorInvalidValue);
     std::lock_guard<std::mutex> lk(g_map_mu);
@@ -204,10 +207,17 @@ int launch_lane_mix_inst(const Typed<T>& t, cudaStream_t stream)
     CUtensorMap mapB, mapC;
     AS_TRY(make_bc_tensor_map<T>(&mapB, t.B, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
     AS_TRY(make_bc_tensor_map<T>(&mapC, t.C, static_cast<int64_t>(t.batch) * 16, t.L, kLaneRowTc, 16));
+    // x and delta as [rows, L] matrices, boxes of {128 bytes, 8 rows}, 128-byte swizzle
+    CUtensorMap mapX, mapD;
+    const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
+    constexpr int kBoxT = 128 / static_cast<int>(sizeof(T));
+    AS_TRY(make_bc_tensor_map<T>(&mapX, t.x, rows, t.L, kBoxT, 8, true));
+    AS_TRY(make_bc_tensor_map<T>(&mapD, t.delta, rows, t.L, kBoxT, 8, true));
     int sms = 0;
     AS_TRY(sm_count(&sms));
     kern<<<static_cast<unsigned>(sms), 16 * 32, smem, stream>>>(
-        t.x, t.delta, t.A, mapB, mapC, t.D, t.h0, t.y, t.h_last, t.ext, t.batch, t.d_inner, t.L);
+        t.x, t.delta, t.A, mapB, mapC, mapX, mapD, t.D, t.h0, t.y, t.h_last, t.ext, t.batch,
+        t.d_inner, t.L);
     return after_launch();
 }
 
@@ -257,7 +267,10 @@ int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
     if (poly16 < 0) poly16 = kLaneRowDefaultPoly16;
     if (G == 3) {   // balanced grid: three G = 2 warps + one G = 4 warp per sub-partition
         if (t.d_inner < 224) return AFFINESCAN_ERR_UNSUPPORTED;
-        if (!t.has_ext) return launch_lane_mix_inst<T, 0, 0, 1>(t, stream);
+#ifndef LR_MIX_ORDER
+#define LR_MIX_ORDER 1
+#endif
+        if (!t.has_ext) return launch_lane_mix_inst<T, 0, 0, LR_MIX_ORDER>(t, stream);
         if (is_gated(t)) return launch_lane_mix_inst<T, 0, kExtGated, 1>(t, stream);
         return launch_lane_mix_inst<T, 0, kExtGeneric, 1>(t, stream);
     }

@@ -166,7 +166,15 @@ struct SharedTiles {
     uint64_t* full;    // [kMixStages], count 1 (producer)
     uint64_t* empty;   // [kMixStages], count = consumer warps with work
     int bsel;          // which of the CTA's batches this warp's rows belong to
+    // x / delta ring of the warp (XTMA): 2 stages x (x rows | delta rows), 128 B per row and stage
+    // = kXGroups 128-bit groups, written by TMA tensor copies with the 128-byte swizzle
+    unsigned char* xring;
+    uint64_t* xfull;   // [2], count 1
+    const CUtensorMap* mapX;
+    const CUtensorMap* mapD;
 };
+constexpr int kXGroups = 8;              // 128-bit groups per row per ring stage
+constexpr int kXPerWarp = 2 * 2 * 16 * 128;  // stages x arrays x rows (<= 16) x 128 B
 
 // The staging duty of the balanced grid: TMA tensor copies of the raw [2N][TC] boxes of the CTA's
 // batches into a two-slot raw ring, widened and transposed (lane j = raw row j) into the ring of
@@ -240,7 +248,7 @@ struct MixStager {
 // LaneRowSmem<T, TC>::kPerWarp bytes and the warp stages its own B/C tiles; SHARED == true: the
 // tiles come from `sh`.
 template <typename T, int G, int TC, int F16, int DEG, int EXT, int ASTR, int ORDER,
-          bool SHARED = false>
+          bool SHARED = false, bool XTMA = false>
 __device__ __forceinline__ void
 lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float* __restrict__ A,
               const CUtensorMap* mapB, const CUtensorMap* mapC, const float* __restrict__ D,
@@ -334,19 +342,64 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
     if (G >= 2) yoff += (g & (G / 2)) ? VEC / 2 : 0;
     if (G >= 4) yoff += (g & 1) ? VEC / 4 : 0;
 
-    // A1: raw 128-bit prefetch, two groups (2*VEC timesteps) ahead
+    // A1 (XTMA): the warp's rows of x and delta come through its own shared-memory ring, one
+    // 128-byte row segment (kXGroups groups) per row and stage, filled by TMA tensor copies of
+    // boxes {128 B, 8 rows} with the 128-byte swizzle: the strided per-row global loads (one L1
+    // wavefront per row and instruction) become two conflict-free LDS.128 per group.
+    static_assert(!XTMA || (SHARED && G >= 2 && kXGroups % (TC / VEC) == 0), "x ring");
+    constexpr int kXRows = 32 / G;
+    constexpr int kXArray = kXRows * 128;
+    constexpr int kXStage = 2 * kXArray;
+    const long long nxblocks = (L + kXGroups * VEC - 1) / (kXGroups * VEC);
+    auto issue_x = [&](long long blk) {
+        if (XTMA && lane == 0) {
+            const int xs = static_cast<int>(blk & 1);
+            const int t0 = static_cast<int>(blk * (kXGroups * VEC));
+            unsigned char* dst = sh.xring + xs * kXStage;
+            mbar_arrive_expect_tx(&sh.xfull[xs], static_cast<unsigned>(kXStage));
+#pragma unroll
+            for (int bx = 0; bx < kXRows / 8; ++bx) {
+                tma_tile_2d_g2s(dst + bx * 1024, sh.mapX, t0, static_cast<int>(row0) + bx * 8,
+                                &sh.xfull[xs]);
+                tma_tile_2d_g2s(dst + kXArray + bx * 1024, sh.mapD, t0,
+                                static_cast<int>(row0) + bx * 8, &sh.xfull[xs]);
+            }
+        }
+    };
+    if (XTMA) {
+        if (lane == 0) {
+            mbar_init(&sh.xfull[0], 1);
+            mbar_init(&sh.xfull[1], 1);
+            fence_mbar_init();
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        issue_x(0);
+        if (nxblocks > 1) issue_x(1);
+    }
+    // this lane's row inside the ring: box (row / 8), line (row % 8), chunks XOR-swizzled by line
+    const int xline = (lane / G) & 7;
+    const int xrowoff = ((lane / G) >> 3) * 1024 + xline * 128;
+
+    // A1 (no XTMA): raw 128-bit prefetch, PD groups (PD*VEC timesteps) ahead
     constexpr int PD = LR_PD;  // 128-bit x/delta groups in flight per row
     uint4 xq[PD], dq[PD];
 #pragma unroll
     for (int i = 0; i < PD; ++i) {
         xq[i] = make_uint4(0, 0, 0, 0);
         dq[i] = make_uint4(0, 0, 0, 0);
-        if (static_cast<long long>(i) * VEC < L) {
+        if (!XTMA && static_cast<long long>(i) * VEC < L) {
             xq[i] = __ldcs(reinterpret_cast<const uint4*>(xr) + i);
             dq[i] = __ldcs(reinterpret_cast<const uint4*>(dr) + i);
         }
     }
 
+    if (XTMA) {  // words of group 0 (chunk 0 of block 0: swizzled position = xline)
+        mbar_wait(&sh.xfull[0], 0u);
+        const unsigned char* p0 = sh.xring + xrowoff + (xline << 4);
+        xq[0] = lds128(p0);
+        dq[0] = lds128(p0 + kXArray);
+    }
     if (SHARED && stg) stg->prologue(lane);
     for (long long tile = 0; tile < ntiles; ++tile) {
         const long long t0 = tile * TC;
@@ -379,6 +432,12 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
         }
 
         // A3..A9: sequential in t.  One group = VEC timesteps of the warp's rows.
+        // x ring: the tile lies inside one ring block
+        const long long xblk = (tile * kChunks) / kXGroups;
+        const int xcb = static_cast<int>((tile * kChunks) % kXGroups);
+        const int xs = static_cast<int>(xblk & 1);
+        const unsigned char* xbase = XTMA ? sh.xring + xs * kXStage + xrowoff : nullptr;
+
         // `fasttag`: the group and its prefetch refill lie inside the row, so every address is the
         // tile's base pointer plus a constant (no 64-bit position arithmetic per group)
         auto group = [&](auto pitag, auto fasttag, const int grp, const long long tg, const T* xg,
@@ -386,9 +445,35 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
             constexpr int PI = decltype(pitag)::value;
             constexpr bool FAST = decltype(fasttag)::value;
             float xv[VEC], dl[VEC];
-            unpack128<T>(xq[PI], xv);
-            unpack128<T>(dq[PI], dl);
-            {   // refill the prefetch slot.  G >= 2 (four warps per sub-partition): always,
+            if (XTMA) {
+                // this group's words were read from the ring one group ago; now read the next
+                // group's (the first group of the next block waits for that block's copies)
+                unpack128<T>(xq[0], xv);
+                unpack128<T>(dq[0], dl);
+                const int c1 = xcb + grp + 1;
+                if (c1 < kXGroups) {
+                    const int chunk = (c1 ^ xline) << 4;
+                    xq[0] = lds128(xbase + chunk);
+                    dq[0] = lds128(xbase + kXArray + chunk);
+                } else {
+                    if (xblk + 1 < nxblocks) {
+                        mbar_wait(&sh.xfull[xs ^ 1], static_cast<unsigned>(((xblk + 1) >> 1) & 1));
+                        const unsigned char* nb = sh.xring + (xs ^ 1) * kXStage + xrowoff + (xline << 4);
+                        xq[0] = lds128(nb);
+                        dq[0] = lds128(nb + kXArray);
+                    }
+                    // every word of this block is in registers: refill its stage
+                    __syncwarp();
+                    if (xblk + 2 < nxblocks) {
+                        fence_proxy_async_smem();
+                        issue_x(xblk + 2);
+                    }
+                }
+            } else {
+                unpack128<T>(xq[PI], xv);
+                unpack128<T>(dq[PI], dl);
+            }
+            if (!XTMA) {   // refill the prefetch slot.  G >= 2 (four warps per sub-partition): always,
                 // past the end of the row this group is re-read and never used (a
                 // conditional refill costs a register copy per word: +2.5 %); G = 1:
                 // conditional (measured: the unconditional form is scheduled late and
@@ -481,9 +566,9 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                     for (int s = 0; s < PP; s += 2) {
                         const int p = PP * q + s;
                         const ulonglong2 b4 =
-                            *reinterpret_cast<const ulonglong2*>(bct + 2 * s);
+                            lds128_u64x2(bct + 2 * s);
                         const ulonglong2 c4 =
-                            *reinterpret_cast<const ulonglong2*>(bct + N + 2 * s);
+                            lds128_u64x2(bct + N + 2 * s);
                         h2[p] = fma2(av[k][s], h2[p], mul2(dxx, b4.x));
                         h2[p + 1] = fma2(av[k][s + 1], h2[p + 1], mul2(dxx, b4.y));
                         y2[k] = fma2(c4.x, h2[p], y2[k]);
@@ -506,9 +591,9 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
                     const bool rs = RST && ((rmask >> k) & 1u);
 #pragma unroll
                     for (int p = 0; p < NP; p += 2) {
-                        const ulonglong2 b4 = *reinterpret_cast<const ulonglong2*>(bct + 2 * p);
+                        const ulonglong2 b4 = lds128_u64x2(bct + 2 * p);
                         const ulonglong2 c4 =
-                            *reinterpret_cast<const ulonglong2*>(bct + N + 2 * p);
+                            lds128_u64x2(bct + N + 2 * p);
                         pair_t a2[2];
 #pragma unroll
                         for (int s = 0; s < 2; ++s) {
@@ -677,10 +762,13 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 template <typename T, int TC>
 struct LaneMixSmem {
     using S = LaneRowSmem<T, TC>;
+    static constexpr int kXBytes = 16 * kXPerWarp;  // x/delta rings of the 16 row warps (first:
+                                                    // the swizzled boxes want 1024-byte alignment)
     static constexpr int kBcBytes = kMixStages * kMixMaxBatches * S::kBcTile;
     static constexpr int kRawBytes = 2 * kMixMaxBatches * S::kRawStage;
-    static constexpr int kBarOffset = kBcBytes + kRawBytes;
-    static constexpr int kBytes = kBarOffset + (2 * kMixStages + 2) * 8 + 64;
+    static constexpr int kBarOffset = kXBytes + kBcBytes + kRawBytes;
+    // full[], empty[], raw_full[2], xfull[16][2]; + 1024 to align the base
+    static constexpr int kBytes = kBarOffset + (2 * kMixStages + 2 + 32) * 8 + 64 + 1024;
 };
 
 template <typename T, int TC, int F16, int DEG, int EXT, int ORDER>
@@ -689,6 +777,8 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
                                const float* __restrict__ A,
                                const __grid_constant__ CUtensorMap mapB,
                                const __grid_constant__ CUtensorMap mapC,
+                               const __grid_constant__ CUtensorMap mapX,
+                               const __grid_constant__ CUtensorMap mapD,
                                const float* __restrict__ D,
                                const float* __restrict__ h0, T* __restrict__ y,
                                float* __restrict__ h_last, const SelectiveExt ext, int batch,
@@ -697,12 +787,18 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
     using M = LaneMixSmem<T, TC>;
     constexpr int kRowsPerCta = 12 * 16 + 4 * 8;
     constexpr int kStagerWarp = 12;  // the first G = 4 warp also stages the CTA's B/C tiles
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    float* bc_ring = reinterpret_cast<float*>(smem_raw);
-    unsigned char* raw_ring = smem_raw + M::kBcBytes;
+    // x / delta through the per-warp TMA ring: plain form only (measured: the fused forms, which
+    // also stream z, lose 6 % with it; the plain form gains 1 % and frees 12 % of the L1 data pipe)
+    constexpr bool kXtma = EXT == 0;
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    unsigned char* smem_raw = reinterpret_cast<unsigned char*>(
+        (reinterpret_cast<uintptr_t>(smem_dyn) + 1023) & ~static_cast<uintptr_t>(1023));
+    float* bc_ring = reinterpret_cast<float*>(smem_raw + M::kXBytes);
+    unsigned char* raw_ring = smem_raw + M::kXBytes + M::kBcBytes;
     uint64_t* full = reinterpret_cast<uint64_t*>(smem_raw + M::kBarOffset);
     uint64_t* empty = full + kMixStages;
     uint64_t* raw_full = empty + kMixStages;
+    uint64_t* xfull = raw_full + 2;  // [16 warps][2]
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -754,17 +850,21 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
         sh.full = full;
         sh.empty = empty;
         sh.bsel = 0;
+        sh.xring = smem_raw + warp * kXPerWarp;
+        sh.xfull = xfull + 2 * warp;
+        sh.mapX = &mapX;
+        sh.mapD = &mapD;
         if (warp < 12) {
             if (warp < n2) {
                 const long long row0 = cta0 + warp * 16;
                 sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
-                lane_row_warp<T, 2, TC, F16, DEG, EXT, 0, ORDER, true>(
+                lane_row_warp<T, 2, TC, F16, DEG, EXT, 0, ORDER, true, kXtma>(
                     x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh);
             }
         } else if (warp - 12 < n4) {
             const long long row0 = cta0 + r2 + (warp - 12) * 8;
             sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
-            lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true>(
+            lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true, kXtma>(
                 x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh,
                 warp == kStagerWarp ? &stager : nullptr);
         } else if (warp == kStagerWarp) {

@@ -366,14 +366,7 @@ lane_row_warp(const T* __restrict__ x, const T* __restrict__ delta, const float*
             }
         }
     };
-    if (XTMA) {
-        if (lane == 0) {
-            mbar_init(&sh.xfull[0], 1);
-            mbar_init(&sh.xfull[1], 1);
-            fence_mbar_init();
-        }
-        fence_proxy_async_smem();
-        __syncwarp();
+    if (XTMA) {  // (the CTA initialised sh.xfull[0..1], count 1)
         issue_x(0);
         if (nxblocks > 1) issue_x(1);
     }
@@ -818,9 +811,9 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
         const int nb = static_cast<int>((cta0 + cta_rows - 1) / d_inner) - b_first + 1;
         __syncthreads();  // previous round's barriers are quiet
         if (threadIdx.x == 0) {
+            // a used mbarrier must be invalidated before it is initialised again
             if (base != 0) {
-#pragma unroll
-                for (int s = 0; s < 2 * kMixStages + 2; ++s) mbar_inval(&full[s]);
+                for (int s = 0; s < 2 * kMixStages + 2 + 32; ++s) mbar_inval(&full[s]);
             }
 #pragma unroll
             for (int s = 0; s < kMixStages; ++s) {
@@ -829,6 +822,7 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
             }
             mbar_init(&raw_full[0], 1);
             mbar_init(&raw_full[1], 1);
+            for (int s = 0; s < 32; ++s) mbar_init(&xfull[s], 1);  // x rings: [warp][2]
             fence_mbar_init();
         }
         fence_proxy_async_smem();

@@ -202,14 +202,16 @@ def test_lane_row_balanced_grid_partial_ctas_rounds_and_fused_steps(cuda_device,
     """OPT_LANE_ROW_G = 3: one CTA per SM, three 16-row warps and one 8-row warp per
     sub-partition, B/C staged once per CTA by a producer warp.  Shapes: a CTA's 224 rows
     straddling two batches, a last CTA with fewer rows than warps, more rows than one round of
-    CTAs holds, L not a multiple of the staged tile; plain, gated and reset forms."""
+    CTAs holds (with few and with many tiles, so that every barrier is re-armed after use), L not a
+    multiple of the staged tile; plain, gated and reset forms."""
     sms = torch.cuda.get_device_properties(cuda_device).multi_processor_count
     vec = 4 if dtype == torch.float32 else 8
     lib.set_option(lib.OPT_LANE_ROW_G, 3)
     try:
         seed = 900
         for (batch, d_inner, L) in [(1, 224, 64), (3, 256, 3 * 32 + vec), (2, 480, 520),
-                                    (1, 224 * sms + 96, 40), (5, 1024, 96 + vec)]:
+                                    (1, 224 * sms + 96, 40), (5, 1024, 96 + vec),
+                                    (2, 224 * sms // 2 + 160, 8 * 64 + vec)]:
             for mode in ("plain", "gated", "reset"):
                 seed += 1
                 inp = _inputs(batch, d_inner, L, dtype, cuda_device, seed, with_h0=(seed % 2 == 0))

@@ -239,6 +239,24 @@ int launch_lane_row_gf(const Typed<T>& t, cudaStream_t stream)
     return launch_lane_row_inst<T, G, F16, kExtGeneric, 0, kOrder>(t, stream);
 }
 
+// Grid of the lane_row schedule from the row count: modelled cycles per timestep
+// on the busiest sub-partition, fitted to the r02 sweeps on B200 (w = row warps resident there).
+// Returns the cost of the best grid; *G = 1 | 2 (lanes per row, uniform grid) | 3 (balanced grid).
+int64_t lane_grid_cost(int64_t rows, int d_inner, int sms, bool wide, int* G)
+{
+    const int64_t smsp = static_cast<int64_t>(sms) * 4;
+    const int64_t w1 = (rows / 32 + smsp - 1) / smsp, w2 = (rows / 16 + smsp - 1) / smsp;
+    const int64_t per_round = static_cast<int64_t>(sms) * 224;
+    const int64_t rounds = (rows + per_round - 1) / per_round;
+    // fp32 io pays more per warp (wider tiles, degree-5 polynomial)
+    const int64_t c1 = wide ? 350 * w1 : (w1 == 1 ? 215 : 40 + 150 * w1);
+    const int64_t c2 = wide ? 20 + 150 * w2 : 45 + 80 * w2;
+    const int64_t c3 = d_inner >= 224 ? (wide ? 335 : 290) * rounds
+                                      : std::numeric_limits<int64_t>::max();
+    *G = (c3 < c1 && c3 < c2) ? 3 : (c2 < c1 ? 2 : 1);
+    return *G == 3 ? c3 : (*G == 2 ? c2 : c1);
+}
+
 template <typename T>
 int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
 {
@@ -251,17 +269,9 @@ int launch_lane_row(const Typed<T>& t, int a_structure, cudaStream_t stream)
     int G = g_opt_lane_row_g.load(std::memory_order_relaxed);
     int poly16 = g_opt_lane_row_poly16.load(std::memory_order_relaxed);
     if (G < 0) {
-        // Grid shape from the row count: cycles per timestep on the busiest
-        // sub-partition, fitted to measurements on B200 (w = resident row warps there).
         int sms = 0;
         AS_TRY(sm_count(&sms));
-        const int64_t rows = static_cast<int64_t>(t.batch) * t.d_inner;
-        const int64_t smsp = static_cast<int64_t>(sms) * 4;
-        const int64_t w1 = (rows / 32 + smsp - 1) / smsp, w2 = (rows / 16 + smsp - 1) / smsp;
-        const int64_t rounds = (rows + static_cast<int64_t>(sms) * 224 - 1) / (static_cast<int64_t>(sms) * 224);
-        const int64_t c1 = 110 + 118 * w1, c2 = 140 + 59 * w2, c3 = 296 * rounds;
-        const bool mix_ok = t.d_inner >= 224;
-        G = (mix_ok && c3 < c1 && c3 < c2) ? 3 : (c2 < c1 ? 2 : 1);
+        lane_grid_cost(static_cast<int64_t>(t.batch) * t.d_inner, t.d_inner, sms, sizeof(T) == 4, &G);
         if (poly16 < 0) poly16 = G == 1 ? kLaneRowDefaultPoly16 : 0;
     }
     if (poly16 < 0) poly16 = kLaneRowDefaultPoly16;
@@ -402,7 +412,14 @@ int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
         // too few rows to give every SM a CTA of row-warps, and at least a few tiles per row:
         // parallelise L across CTAs with the decoupled look-back carry
         const bool few_rows = rows * 2 < static_cast<int64_t>(sms) * kWarpRowTmaMaxWarps;
-        if (lane_ok && rows >= lane_row_min_rows) variant = AFFINESCAN_SELECTIVE_LANE_ROW;
+        // general A: lanes = rows (sequential in L) against lanes = timesteps (warp_row_tma, measured
+        // ~3.03 cycles per timestep per row and SM): whichever the model says is faster
+        int g_unused = 0;
+        const bool lane_wins =
+            a.a_structure != AFFINESCAN_A_GENERAL
+                ? rows >= lane_row_min_rows
+                : lane_grid_cost(rows, t.d_inner, sms, sizeof(T) == 4, &g_unused) * sms < 3 * rows;
+        if (lane_ok && lane_wins) variant = AFFINESCAN_SELECTIVE_LANE_ROW;
         else if (tma_ok && few_rows && t.L >= kChunkedMinL) variant = AFFINESCAN_SELECTIVE_CHUNKED;
         else if (tma_ok && t.L >= kWarpRowTmaMinL) variant = AFFINESCAN_SELECTIVE_WARP_ROW_TMA;
         else variant = AFFINESCAN_SELECTIVE_WARP_ROW;

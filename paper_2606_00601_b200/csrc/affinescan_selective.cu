@@ -194,6 +194,27 @@ int launch_lane_row_inst(const Typed<T>& t, cudaStream_t stream)
     return after_launch();
 }
 
+// Composition of the balanced grid for `rows` rows: the rows are cut into the fewest rounds of at
+// most 224 rows per SM, and a round gives every sub-partition u units of 8 rows (u <= 7) as q2
+// two-lane warps (2 units) and q4 four-lane warps (1 unit).
+// Returns the number of rounds.
+int64_t lane_mix_shape(int64_t rows, int sms, int* q2, int* q4, int* units = nullptr)
+{
+    const int64_t cap = static_cast<int64_t>(sms) * 224;
+    const int64_t rounds = rows <= 0 ? 1 : (rows + cap - 1) / cap;
+    const int64_t per_sm = (rows + rounds * sms - 1) / (rounds * sms);
+    int u = static_cast<int>((per_sm + 31) / 32);
+    u = u < 1 ? 1 : (u > 7 ? 7 : u);
+    // measured best composition per u (r02 sweep): four-lane warps pay twice the per-timestep
+    // work per row, but a sub-partition wants two or three warps to hide latencies
+    static const int kQ2[8] = {0, 0, 0, 1, 1, 2, 3, 3};
+    static const int kQ4[8] = {0, 1, 2, 1, 2, 1, 0, 1};
+    *q2 = kQ2[u];
+    *q4 = kQ4[u];
+    if (units) *units = u;
+    return rounds;
+}
+
 template <typename T, int F16, int EXT, int ORDER>
 int launch_lane_mix_inst(const Typed<T>& t, cudaStream_t stream)
 {
@@ -215,9 +236,11 @@ int launch_lane_mix_inst(const Typed<T>& t, cudaStream_t stream)
     AS_TRY(make_bc_tensor_map<T>(&mapD, t.delta, rows, t.L, kBoxT, 8, true));
     int sms = 0;
     AS_TRY(sm_count(&sms));
+    int q2 = 0, q4 = 0;
+    lane_mix_shape(rows, sms, &q2, &q4);
     kern<<<static_cast<unsigned>(sms), 16 * 32, smem, stream>>>(
         t.x, t.delta, t.A, mapB, mapC, mapX, mapD, t.D, t.h0, t.y, t.h_last, t.ext, t.batch,
-        t.d_inner, t.L);
+        t.d_inner, t.L, q2, q4);
     return after_launch();
 }
 
@@ -246,12 +269,15 @@ int64_t lane_grid_cost(int64_t rows, int d_inner, int sms, bool wide, int* G)
 {
     const int64_t smsp = static_cast<int64_t>(sms) * 4;
     const int64_t w1 = (rows / 32 + smsp - 1) / smsp, w2 = (rows / 16 + smsp - 1) / smsp;
-    const int64_t per_round = static_cast<int64_t>(sms) * 224;
-    const int64_t rounds = (rows + per_round - 1) / per_round;
+    int q2 = 0, q4 = 0, u = 0;
+    const int64_t rounds = lane_mix_shape(rows, sms, &q2, &q4, &u);
     // fp32 io pays more per warp (wider tiles, degree-5 polynomial)
     const int64_t c1 = wide ? 350 * w1 : (w1 == 1 ? 215 : 40 + 150 * w1);
-    const int64_t c2 = wide ? 20 + 150 * w2 : 45 + 80 * w2;
-    const int64_t c3 = d_inner >= 224 ? (wide ? 335 : 290) * rounds
+    const int64_t c2 = wide ? 20 + 150 * w2 : (w2 == 1 ? 143 : 45 + 80 * w2);
+    // balanced grid: cost of a round by units of 8 rows per sub-partition
+    static const int kMix16[8] = {0, 126, 155, 189, 206, 236, 288, 290};
+    static const int kMix32[8] = {0, 161, 189, 236, 232, 283, 338, 332};
+    const int64_t c3 = d_inner >= 224 ? (wide ? kMix32[u] : kMix16[u]) * rounds
                                       : std::numeric_limits<int64_t>::max();
     *G = (c3 < c1 && c3 < c2) ? 3 : (c2 < c1 ? 2 : 1);
     return *G == 3 ? c3 : (*G == 2 ? c2 : c1);
@@ -413,12 +439,19 @@ int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
         // parallelise L across CTAs with the decoupled look-back carry
         const bool few_rows = rows * 2 < static_cast<int64_t>(sms) * kWarpRowTmaMaxWarps;
         // general A: lanes = rows (sequential in L) against lanes = timesteps (warp_row_tma, measured
-        // ~3.03 cycles per timestep per row and SM): whichever the model says is faster
+        // ~3.03 cycles per timestep per row and SM, over whole warp tiles of 32 K timesteps):
+        // whichever the model says is faster (lane_row only when clearly so: warp_row_tma's cost
+        // is not linear in the row count below a few CTAs per SM)
         int g_unused = 0;
-        const bool lane_wins =
-            a.a_structure != AFFINESCAN_A_GENERAL
-                ? rows >= lane_row_min_rows
-                : lane_grid_cost(rows, t.d_inner, sms, sizeof(T) == 4, &g_unused) * sms < 3 * rows;
+        bool lane_wins = rows >= lane_row_min_rows;
+        if (a.a_structure == AFFINESCAN_A_GENERAL && lane_ok) {
+            const int64_t tile_t = TmaShape<T>::S::kTileT;
+            const int64_t padded = (t.L + tile_t - 1) / tile_t * tile_t;
+            const double c_tma = 3.03 * static_cast<double>(rows) / sms *
+                                     (static_cast<double>(padded) / static_cast<double>(t.L)) + 8.0;
+            lane_wins = static_cast<double>(lane_grid_cost(rows, t.d_inner, sms, sizeof(T) == 4,
+                                                           &g_unused)) < 0.85 * c_tma;
+        }
         if (lane_ok && lane_wins) variant = AFFINESCAN_SELECTIVE_LANE_ROW;
         else if (tma_ok && few_rows && t.L >= kChunkedMinL) variant = AFFINESCAN_SELECTIVE_CHUNKED;
         else if (tma_ok && t.L >= kWarpRowTmaMinL) variant = AFFINESCAN_SELECTIVE_WARP_ROW_TMA;

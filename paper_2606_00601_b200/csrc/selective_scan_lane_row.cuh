@@ -742,11 +742,12 @@ selective_scan_lane_row_kernel(const T* __restrict__ x, const T* __restrict__ de
 // ====================================================================================
 // Balanced grid (one CTA of 16 row warps per SM): the XU pipe of a sub-partition
 // is the wall, and with R rows the uniform grid leaves sub-partitions holding ceil(...) warps
-// next to ones holding floor(...).  Here every sub-partition gets three G = 2 warps (16 rows
-// each) and one G = 4 warp (8 rows): 56 rows = 7/8 of what two G = 1 warps carry, spread over
-// four warps whose MUFU, fma and LDS instructions interleave.  Warp w of a CTA runs on
-// sub-partition w % 4.  CTA c owns rows [224 c, 224 c + 224) of a round (rounds of grid * 224
-// rows): the first 192 go to the G = 2 warps, the last 32 to the G = 4 warps.  Those rows lie in
+// next to ones holding floor(...).  Here every sub-partition gets q2 G = 2 warps (16 rows each)
+// and q4 G = 4 warps (8 rows), chosen by the host from the row count; for cfg3 three and one:
+// 56 rows = 7/8 of what two G = 1 warps carry, spread over four warps whose MUFU, fma and LDS
+// instructions interleave.  Warp w of a CTA runs on sub-partition w % 4.  CTA c owns rows
+// [R c, R c + R) of a round, R = 64 q2 + 32 q4 (rounds of grid * R rows): the first 64 q2 go to
+// the G = 2 warps, the rest to the G = 4 warps.  Those rows lie in
 // at most kMixMaxBatches batches (the launcher checks d_inner), whose B/C tiles one of the
 // G = 4 warps (MixStager) stages ONCE for the whole CTA, kMixStages - 1 tiles ahead of its own row work: TMA tensor copies of the raw [2N][TC] boxes into a
 // two-slot raw ring, widened and transposed into a kMixStages-deep ring of fp32 [TC][2][N]
@@ -775,11 +776,15 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
                                const float* __restrict__ D,
                                const float* __restrict__ h0, T* __restrict__ y,
                                float* __restrict__ h_last, const SelectiveExt ext, int batch,
-                               int d_inner, long long L)
+                               int d_inner, long long L, int q2, int q4)
 {
     using M = LaneMixSmem<T, TC>;
-    constexpr int kRowsPerCta = 12 * 16 + 4 * 8;
-    constexpr int kStagerWarp = 12;  // the first G = 4 warp also stages the CTA's B/C tiles
+    // composition of every sub-partition: q2 G = 2 warps (16 rows) and q4 G = 4 warps (8 rows),
+    // q2 + q4 <= 4; warp w = slot * 4 + sub-partition.  The CTA's rows: 64 q2 for the G = 2 warps,
+    // then 32 q4 for the G = 4 warps.
+    const int kRowsPerCta = 64 * q2 + 32 * q4;
+    // the last slot's warp on sub-partition 0 also stages the CTA's B/C tiles
+    const int kStagerWarp = (q2 + q4 - 1) * 4;
     // x / delta through the per-warp TMA ring: plain form only (measured: the fused forms, which
     // also stream z, lose 6 % with it; the plain form gains 1 % and frees 12 % of the L1 data pipe)
     constexpr bool kXtma = EXT == 0;
@@ -804,9 +809,10 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
         if (cta0 >= rows) break;  // CTA-uniform
         const long long cta_rows = rows - cta0 < kRowsPerCta ? rows - cta0 : kRowsPerCta;
         // rows of this CTA: G = 2 warps take 16 each from the front, G = 4 warps 8 each after them
-        const long long r2 = cta_rows < 192 ? (cta_rows / 16) * 16 : 192;
+        // (cta_rows % 32 == 0)
+        const long long r2 = cta_rows < 64 * q2 ? cta_rows : 64 * q2;
         const int n2 = static_cast<int>(r2 / 16);
-        const int n4 = static_cast<int>((cta_rows - r2 + 7) / 8);  // <= 4 (cta_rows % 8 == 0)
+        const int n4 = static_cast<int>((cta_rows - r2) / 8);
         const int b_first = static_cast<int>(cta0 / d_inner);
         const int nb = static_cast<int>((cta0 + cta_rows - 1) / d_inner) - b_first + 1;
         __syncthreads();  // previous round's barriers are quiet
@@ -848,20 +854,31 @@ selective_scan_lane_mix_kernel(const T* __restrict__ x, const T* __restrict__ de
         sh.xfull = xfull + 2 * warp;
         sh.mapX = &mapX;
         sh.mapD = &mapD;
-        if (warp < 12) {
-            if (warp < n2) {
-                const long long row0 = cta0 + warp * 16;
+        const int slot = warp >> 2, sp = warp & 3;
+        const MixStager<T, TC>* stg = warp == kStagerWarp ? &stager : nullptr;
+        bool worked = false;
+        if (slot < q2) {
+            const int i2 = slot * 4 + sp;
+            if (i2 < n2) {
+                const long long row0 = cta0 + i2 * 16;
                 sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
                 lane_row_warp<T, 2, TC, F16, DEG, EXT, 0, ORDER, true, kXtma>(
-                    x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh);
+                    x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh,
+                    stg);
+                worked = true;
             }
-        } else if (warp - 12 < n4) {
-            const long long row0 = cta0 + r2 + (warp - 12) * 8;
-            sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
-            lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true, kXtma>(
-                x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh,
-                warp == kStagerWarp ? &stager : nullptr);
-        } else if (warp == kStagerWarp) {
+        } else if (slot < q2 + q4) {
+            const int i4 = (slot - q2) * 4 + sp;
+            if (i4 < n4) {
+                const long long row0 = cta0 + r2 + i4 * 8;
+                sh.bsel = static_cast<int>(row0 / d_inner) - b_first;
+                lane_row_warp<T, 4, TC, F16, DEG, EXT, 0, ORDER, true, kXtma>(
+                    x, delta, A, &mapB, &mapC, D, h0, y, h_last, ext, d_inner, L, row0, nullptr, sh,
+                    stg);
+                worked = true;
+            }
+        }
+        if (stg && !worked) {
             // a last CTA without rows for this warp: staging only
             stager.issue_raw(0, lane);
             if (ntiles > 1) stager.issue_raw(1, lane);

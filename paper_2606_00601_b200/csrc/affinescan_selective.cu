@@ -435,9 +435,12 @@ int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
         // one row per FP32 lane of the machine; the structured-A paths need far
         // fewer instructions per row-step, so they pay off from one warp per sub-partition
         const int64_t lane_row_min_rows = static_cast<int64_t>(sms) * 128;
-        // too few rows to give every SM a CTA of row-warps, and at least a few tiles per row:
-        // parallelise L across CTAs with the decoupled look-back carry
-        const bool few_rows = rows * 2 < static_cast<int64_t>(sms) * kWarpRowTmaMaxWarps;
+        // very few rows and at least a few tiles per row: parallelise L across CTAs with the
+        // decoupled look-back carry.  CHUNKED pays a second exp per state-step, so its time grows
+        // with rows * L (~3.3e-8 ms per element) while warp_row_tma's is the serial chain of a
+        // row's tiles (~2.7 us each) as long as the rows fit one wave: measured crossover at
+        // ~200 rows on 148 SMs (64 rows x 2^20: 2.65 against 7.39 ms; 256 x 2^16: 0.58 against 0.48)
+        const bool few_rows = rows * 148 <= static_cast<int64_t>(sms) * 192;
         // general A: lanes = rows (sequential in L) against lanes = timesteps (warp_row_tma, measured
         // ~3.03 cycles per timestep per row and SM, over whole warp tiles of 32 K timesteps):
         // whichever the model says is faster (lane_row only when clearly so: warp_row_tma's cost

@@ -111,16 +111,28 @@ int affine_dispatch(const void* a_, const void* u_, const float* h0, void* h_, f
     // CTAs => carry in a register; otherwise split the flattened stream over tiles with the
     // decoupled look-back carry.  Thresholds scale with the SM count of the device.
     if (variant == AFFINESCAN_VARIANT_AUTO) {
+        // DESIGN.md §6.6, from the r02 sweeps (2^20 .. 2^30 elements, S = 1 .. 2^22, both dtypes).
+        // The persistent look-back stream costs the same whatever the segmentation once a tile
+        // lies inside a sequence; one CTA (or warp) per sequence wins a few percent when there are
+        // several waves of sequences of moderate length; very short sequences leave most lanes of
+        // a per-sequence warp idle, so the flattened stream wins again.
         int sms = 0;
         AS_TRY(sm_count(&sms));
-        const int64_t cta_loop_min_seq = static_cast<int64_t>(sms) * 16;  // >= 4 waves of 4 CTAs / SM:
-                                                                          // fewer leave a ragged last wave
-        const int64_t warp_seq_min_seq = static_cast<int64_t>(sms) * 64;  // >= 64 warps / SM
-        if (num_seq >= cta_loop_min_seq && L >= kAffCtaLoopMinL)
-            variant = AFFINESCAN_AFFINE_CTA_LOOP;
-        else if (num_seq >= warp_seq_min_seq) variant = AFFINESCAN_AFFINE_WARP_SEQ;
-        else if (L <= kAffCtaLoopMinL) variant = AFFINESCAN_AFFINE_CTA_LOOP;  // latency-bound
-        else variant = AFFINESCAN_AFFINE_LOOKBACK;
+        const bool narrow = sizeof(T) == 2;
+        const int64_t waves16 = static_cast<int64_t>(sms) * 16;  // four waves of 4 CTAs per SM
+        if (L <= (narrow ? 512 : 128))
+            variant = num_seq * L >= (1 << 16) ? AFFINESCAN_AFFINE_LOOKBACK : AFFINESCAN_AFFINE_CTA_LOOP;
+        else if (L <= 2048)
+            variant = AFFINESCAN_AFFINE_CTA_LOOP;  // one warp per sequence, no scratch, no ticket
+        else if (narrow)
+            variant = L >= 16384                          ? AFFINESCAN_AFFINE_LOOKBACK
+                      : num_seq >= static_cast<int64_t>(sms) * 8 ? AFFINESCAN_AFFINE_WARP_SEQ
+                      : L <= kAffCtaLoopMinL              ? AFFINESCAN_AFFINE_CTA_LOOP
+                                                          : AFFINESCAN_AFFINE_LOOKBACK;
+        else
+            variant = (L < (1 << 17) && num_seq >= waves16) ? AFFINESCAN_AFFINE_CTA_LOOP
+                      : L <= kAffCtaLoopMinL                ? AFFINESCAN_AFFINE_CTA_LOOP
+                                                            : AFFINESCAN_AFFINE_LOOKBACK;
     }
     int st;
     switch (variant) {

@@ -511,11 +511,12 @@ def test_config5_affine_bandwidth_sweep_every_element(cuda_device):
         lib.affine_scan_ex(a_flat.view(S, L), u_flat.view(S, L), h0_all[:S], h, hl, variant)
         torch.cuda.synchronize()
         if variant == lib.VARIANT_AUTO:
-            # many short sequences => one warp each; long ones => one CTA each while there are
-            # at least four full waves of them, else the persistent look-back stream
+            # fp32 io: up to 2048 steps one single-warp CTA per sequence; longer
+            # ones a CTA each while they are shorter than 2^17 and fill four waves; else the
+            # persistent look-back stream
             sms = torch.cuda.get_device_properties(cuda_device).multi_processor_count
-            want = (lib.AFFINE_WARP_SEQ if L < 8192 else
-                    lib.AFFINE_CTA_LOOP if S >= 16 * sms else lib.AFFINE_LOOKBACK)
+            want = (lib.AFFINE_CTA_LOOP if L <= 2048 or (L < (1 << 17) and S >= 16 * sms)
+                    else lib.AFFINE_LOOKBACK)
             assert lib.last_variant() == want
         outs.append((L, S, variant, h, hl))
     h0_host = h0_all.double().cpu().numpy()

@@ -432,6 +432,27 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
         }
     } else {
         // ------------------------------------------------------------ consumer warps
+        // Short sequences that divide the tile: every tile starts at a head (no carry between
+        // tiles) and a thread's vectors sit at the same place of a sequence in every tile, so the
+        // head / tail flags and the sequence index inside the tile are computed once.
+        const bool aligned_seq = L < kTile && (kTile % static_cast<int>(L)) == 0;
+        unsigned seqmeta = 0;          // bit j: vector j starts a sequence; bit 8 + j: it ends one
+        unsigned slocp[(J + 1) / 2];   // sequence index inside the tile of vector j, 16 bits each
+#pragma unroll
+        for (int j = 0; j < (J + 1) / 2; ++j) slocp[j] = 0;
+#pragma unroll
+        for (int j = 0; j < J; ++j) {
+            if (aligned_seq) {
+                const unsigned off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                const unsigned Lu = static_cast<unsigned>(L);
+                const unsigned sl = off / Lu;
+                const unsigned t = off - sl * Lu;
+                slocp[j / 2] |= sl << (16 * (j & 1));
+                if (t == 0) seqmeta |= 1u << j;
+                if (t + VEC == Lu) seqmeta |= 1u << (8 + j);
+            }
+        }
+        auto sloc_of = [&](int j) { return static_cast<int>((slocp[j / 2] >> (16 * (j & 1))) & 0xffffu); };
         // state of the tile between its A and B phases
         Pair p_excl[J], p_tot[J];
         long long p_tile = -1, p_q0 = 0, p_r0 = 0;
@@ -456,7 +477,25 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
                 // interior tile (the common case): whole tile inside one sequence and inside the
                 // stream, so a head can only sit at offset 0 and a tail at the tile's end
                 const bool fast = (r0 + kTile <= L) && (base + kTile <= total);
-                if (fast) {
+                if (aligned_seq && base + kTile <= total) {
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                        unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), r.av[j]);
+                        unpack128<T>(*reinterpret_cast<const uint4*>(su + off), r.uv[j]);
+                        if ((seqmeta >> j) & 1u) {
+                            const float hin = h0 ? __ldg(h0 + q0 + sloc_of(j)) : 0.0f;
+                            r.uv[j][0] = fmaf(r.av[j][0], hin, r.uv[j][0]);
+                            r.av[j][0] = 0.0f;
+                        }
+                    }
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        row_scan(r, j, lane);
+                        c_excl[j] = r.excl[j];
+                        c_tot[j] = r.tot[j];
+                    }
+                } else if (fast) {
 #pragma unroll
                     for (int j = 0; j < J; ++j) {
                         const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
@@ -535,7 +574,26 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
                 const T* sa = reinterpret_cast<const T*>(smem_raw + p_st * S::kStageBytes);
                 const T* su = sa + kTile;
                 const bool fast = (p_r0 + kTile <= L) && (pbase + kTile <= total);
-                if (fast) {
+                if (aligned_seq && pbase + kTile <= total) {
+#pragma unroll
+                    for (int j = 0; j < J; ++j) {
+                        const int off = warp * kWarpElems + j * 32 * VEC + lane * VEC;
+                        float av[VEC], uv[VEC];
+                        unpack128<T>(*reinterpret_cast<const uint4*>(sa + off), av);
+                        unpack128<T>(*reinterpret_cast<const uint4*>(su + off), uv);
+                        float hs = apply(p_excl[j], H);
+                        if ((seqmeta >> j) & 1u) hs = h0 ? __ldg(h0 + p_q0 + sloc_of(j)) : 0.0f;
+                        float out[VEC];
+#pragma unroll
+                        for (int k = 0; k < VEC; ++k) {
+                            hs = fmaf(av[k], hs, uv[k]);
+                            out[k] = hs;
+                        }
+                        Acc::store(h + pbase + off, out);
+                        if (((seqmeta >> (8 + j)) & 1u) && h_last) h_last[p_q0 + sloc_of(j)] = hs;
+                        H = apply(p_tot[j], H);
+                    }
+                } else if (fast) {
                     const bool tail = (p_r0 + kTile == L);
 #pragma unroll
                     for (int j = 0; j < J; ++j) {

@@ -120,19 +120,28 @@ int affine_dispatch(const void* a_, const void* u_, const float* h0, void* h_, f
         AS_TRY(sm_count(&sms));
         const bool narrow = sizeof(T) == 2;
         const int64_t waves16 = static_cast<int64_t>(sms) * 16;  // four waves of 4 CTAs per SM
-        if (L <= (narrow ? 512 : 128))
-            variant = num_seq * L >= (1 << 16) ? AFFINESCAN_AFFINE_LOOKBACK : AFFINESCAN_AFFINE_CTA_LOOP;
-        else if (L <= 2048)
-            variant = AFFINESCAN_AFFINE_CTA_LOOP;  // one warp per sequence, no scratch, no ticket
-        else if (narrow)
-            variant = L >= 16384                          ? AFFINESCAN_AFFINE_LOOKBACK
-                      : num_seq >= static_cast<int64_t>(sms) * 8 ? AFFINESCAN_AFFINE_WARP_SEQ
-                      : L <= kAffCtaLoopMinL              ? AFFINESCAN_AFFINE_CTA_LOOP
-                                                          : AFFINESCAN_AFFINE_LOOKBACK;
-        else
-            variant = (L < (1 << 17) && num_seq >= waves16) ? AFFINESCAN_AFFINE_CTA_LOOP
-                      : L <= kAffCtaLoopMinL                ? AFFINESCAN_AFFINE_CTA_LOOP
-                                                            : AFFINESCAN_AFFINE_LOOKBACK;
+        // sequences that divide the look-back tile take its aligned path (no carry, flags computed
+        // once per thread): as fast as interior tiles
+        const int64_t lb_tile = kAffLookbackWarps * 32 * kVec * kAffLookbackJ;
+        const bool aligned = vec_ok && L < lb_tile && lb_tile % L == 0;
+        const bool tiny = num_seq * L < (1 << 16);
+        if (narrow) {
+            if (L >= 16384 || ((aligned || L <= 512) && !tiny)) variant = AFFINESCAN_AFFINE_LOOKBACK;
+            else if (L <= 2048) variant = AFFINESCAN_AFFINE_CTA_LOOP;  // one warp per sequence
+            else
+                variant = num_seq >= static_cast<int64_t>(sms) * 8 ? AFFINESCAN_AFFINE_WARP_SEQ
+                          : L <= kAffCtaLoopMinL                   ? AFFINESCAN_AFFINE_CTA_LOOP
+                                                                   : AFFINESCAN_AFFINE_LOOKBACK;
+        } else {
+            if (L <= 256) variant = tiny ? AFFINESCAN_AFFINE_CTA_LOOP : AFFINESCAN_AFFINE_LOOKBACK;
+            else if (L <= 1024) variant = AFFINESCAN_AFFINE_CTA_LOOP;  // one warp per sequence
+            else if (L < 4096)
+                variant = (aligned && !tiny) ? AFFINESCAN_AFFINE_LOOKBACK : AFFINESCAN_AFFINE_CTA_LOOP;
+            else
+                variant = (L < (1 << 17) && num_seq >= waves16) ? AFFINESCAN_AFFINE_CTA_LOOP
+                          : L <= kAffCtaLoopMinL                ? AFFINESCAN_AFFINE_CTA_LOOP
+                                                                : AFFINESCAN_AFFINE_LOOKBACK;
+        }
     }
     int st;
     switch (variant) {

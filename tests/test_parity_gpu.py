@@ -83,6 +83,23 @@ def test_affine_prefix_sum_exact_through_the_whole_carry_chain(cuda_device, vari
     assert np.array_equal(to_f64_numpy(h[:, :4096]), href)
 
 
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_affine_lookback_sequences_that_divide_the_tile(cuda_device, dtype):
+    """Short sequences whose length divides the look-back tile take its aligned path (every tile
+    starts at a head; head / tail flags computed once per thread).  a≡1, u in {0,1}: every prefix
+    is an exact small integer in the fp32 state, so h (rounded once to the io dtype) and h_last must
+    match bitwise, h0 included."""
+    for L in (8, 64, 512, 2048):
+        S = 3 * 8192 // L * 5 + 7                       # many tiles and a ragged last one
+        u = (uniform((S, L), 0, 1, seed=L, stream=0, device=cuda_device) > 0.5).to(dtype)
+        h0 = (uniform((S,), 0, 1, seed=L, stream=1, device=cuda_device) * 8).floor().to(torch.float32)
+        inp = {"a": torch.ones_like(u), "u": u, "h0": h0}
+        h, h_last = gpu_affine(inp, lib.AFFINE_LOOKBACK)
+        ref = h0.double()[:, None] + torch.cumsum(u.double(), dim=1)   # exact in the fp32 state
+        assert torch.equal(h.double(), ref.to(dtype).double()), f"L={L} {dtype}"  # one RNE to io
+        assert torch.equal(h_last.double(), ref[:, -1]), f"L={L} {dtype} h_last"
+
+
 def test_affine_running_product_and_geometric(cuda_device):
     """u≡0 gives h0*prod(a) (a=0.5: exact powers of two until underflow); constant a,u gives
     the geometric series (BJ closed forms), here against the closed form itself."""

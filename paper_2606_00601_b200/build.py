@@ -1,6 +1,9 @@
 """Builds libaffinescan.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2606_00601_b200.build [--force] [--verbose]
+
+AFFINESCAN_NVCC_FLAGS (environment) is appended to the compile flags: the kernels' compile-time tuning
+knobs (-DLR_PD=, -DLR_MIX_STAGES=, -DLR_TC=, -DLR_MIX_ORDER=; defaults in csrc/) for ablation builds.
 """
 from __future__ import annotations
 

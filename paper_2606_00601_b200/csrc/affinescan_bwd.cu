@@ -55,13 +55,7 @@ int bwd_launch(const BwdArgs& a, cudaStream_t stream)
     float* dD_part = dA_part + n_da;
     auto kern = selective_scan_bwd_kernel<T>;
     constexpr int smem = kBwdSmemPerWarp * kBwdWarps;
-    static bool configured[64] = {};
-    int dev = 0;
-    AS_CUDA(cudaGetDevice(&dev));
-    if (!configured[dev & 63]) {  // benign race: the attribute call is idempotent
-        AS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        configured[dev & 63] = true;
-    }
+    AS_TRY(allow_dynamic_smem(reinterpret_cast<const void*>(kern), smem));
     const int64_t blocks = (groups + kBwdWarps - 1) / kBwdWarps;
     if (blocks > 0x7fffffffLL || a.L / 32 + 1 > 0x7fffffffLL) return AFFINESCAN_ERR_UNSUPPORTED;
     kern<<<static_cast<unsigned>(blocks), kBwdWarps * 32, smem, stream>>>(

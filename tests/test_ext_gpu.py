@@ -372,6 +372,47 @@ def test_two_host_threads_on_two_streams_run_concurrently(cuda_device):
             assert_close(h, href, torch.float32, f"thread {i} affine h")
 
 
+def test_persistent_kernels_on_two_streams_share_the_gpu_without_deadlock(cuda_device):
+    """The persistent look-back stream and the balanced lane grid launch one or two CTAs per SM and
+    wait inside the kernel (tile descriptors, mbarriers).  Two such launches on two streams compete
+    for the SMs, so part of each grid may not be resident while the rest runs: tickets are handed
+    to running CTAs only, so both must finish, with the same bits as when run alone."""
+    dev = cuda_device
+    S, L = 3, 6_000_000
+    a = uniform((S, L), 0.99, 1.0, seed=5, stream=1, device=dev, dtype=torch.float32)
+    u = normal((S, L), seed=5, stream=2, device=dev, dtype=torch.float32)
+    inp = _inputs(4, 4096, 512, torch.bfloat16, dev, 11, with_h0=False)
+    def affine(stream):
+        h = torch.empty_like(a); hl = torch.empty(S, device=dev)
+        lib.affine_scan_ex(a, u, None, h, hl, lib.AFFINE_CTA_LOOP if stream is None else lib.AFFINE_LOOKBACK,
+                           stream)
+        return h, hl
+    def selective(stream):
+        y = torch.empty_like(inp["x"]); hl = torch.empty((4, 4096, 16), device=dev)
+        lib.selective_scan_fwd_ex(inp["x"], inp["delta"], inp["A"], inp["B"], inp["C"], inp["D"], None,
+                                  y, hl, lib.SELECTIVE_LANE_ROW, stream)
+        return y, hl
+    lib.set_option(lib.OPT_LANE_ROW_G, 3)
+    try:
+        s1, s2 = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+        torch.cuda.synchronize()
+        h_alone, _ = affine(s1); torch.cuda.synchronize()
+        y_alone, hl_alone = selective(s2); torch.cuda.synchronize()
+        outs = []
+        for _ in range(4):                       # interleave launches on the two streams
+            outs.append((affine(s1), selective(s2), affine(s2), selective(s1)))
+        torch.cuda.synchronize()
+        h_ref, _ = affine(None); torch.cuda.synchronize()
+        for (ha, _), (ys, hls), (hb, _), (yt, hlt) in outs:
+            for h in (ha, hb):                   # look-back: reproducible up to fp association
+                assert rel_err(h, to_f64_numpy(h_ref)) <= 1e-4 and rel_err(h, to_f64_numpy(h_alone)) <= 1e-4
+            assert torch.equal(ys, y_alone) and torch.equal(hls, hl_alone)
+            assert torch.equal(yt, y_alone) and torch.equal(hlt, hl_alone)
+    finally:
+        lib.set_option(lib.OPT_LANE_ROW_G, -1)
+
+
+
 def test_host_entry_point_with_L_zero_writes_h_last(cuda_device):
     """the `_host` form promises the same computation as the device form."""
     inp = _inputs(2, 32, 8, torch.float32, cuda_device, 5)

@@ -311,11 +311,11 @@ def test_selective_lane_row_polynomial_exp_slow_and_fast_decay(cuda_device, lane
     """The fma-pipe 2^x must keep 1 - a accurate when a is close to 1 (tiny delta*|A|: long
     memory) and must flush cleanly when delta*|A| is huge (a underflows): DESIGN.md §7."""
     lib.set_option(lib.OPT_LANE_ROW_POLY16, 4)
-    for G in (1, 2):
+    for G in (1, 2, 3):      # (only G = 1 evaluates part of the 2^x by the polynomial)
         lib.set_option(lib.OPT_LANE_ROW_G, G)
         for shift, a_scale in ((-7.0, 1.0), (-4.0, 0.05), (3.0, 40.0), (5.0, 400.0)):
-            inp = _selective_inputs(1, 64, 16, 1024, dtype, cuda_device, 77, with_h0=True,
-                                    delta_shift=shift)
+            inp = _selective_inputs(1, 64 if G < 3 else 256, 16, 1024, dtype, cuda_device, 77,
+                                    with_h0=True, delta_shift=shift)
             inp["A"] = (inp["A"] * a_scale).contiguous()
             check_selective(inp, lib.SELECTIVE_LANE_ROW,
                             f"lane_row G{G} poly4 shift{shift} Ax{a_scale} {dtype}")

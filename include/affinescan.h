@@ -58,8 +58,10 @@ typedef enum affinescan_status {
     AFFINESCAN_ERR_DTYPE = 3,       /* io_dtype is not an affinescan_dtype                */
     AFFINESCAN_ERR_UNSUPPORTED = 4, /* N outside [1, AFFINESCAN_MAX_N]; unknown variant;
                                        a forced variant that cannot run this shape        */
-    AFFINESCAN_ERR_CUDA = 5         /* a CUDA runtime call failed; see
+    AFFINESCAN_ERR_CUDA = 5,        /* a CUDA runtime call failed; see
                                        affinescan_last_cuda_error()                       */
+    AFFINESCAN_ERR_TOO_LARGE = 6    /* the problem needs more scratch than the fixed array of
+                                       affine_scan_static_scratch holds                   */
 } affinescan_status;
 
 typedef enum affinescan_dtype {
@@ -152,6 +154,52 @@ AFFINESCAN_API int affine_scan_ex(const void* a, const void* u, const float* h0,
 AFFINESCAN_API int affine_scan_host(const void* a, const void* u, const float* h0, void* h,
                                     float* h_last, int64_t num_seq, int64_t L, int io_dtype,
                                     void* cuda_stream);
+
+/* ------------------------------------------------------------------------------------
+ * affine_scan_static_scratch — affine_scan (same arguments, same result as
+ * affine_scan_ex(..., AFFINESCAN_AFFINE_LOOKBACK, ...)) for callers that cannot allocate device
+ * memory.
+ *
+ * Why it exists.  The look-back scan needs one 16-byte descriptor per tile for the carry that
+ * crosses tiles (prefix compositions under P:90 Eq.7).  affine_scan takes that scratch
+ * from cudaMallocAsync.  That is not acceptable everywhere: an inference server that gave all
+ * free HBM to its own cache at start-up has nothing left for the driver to hand out; a framework
+ * whose allocator must own every byte cannot have a library allocate behind its back; a
+ * latency-bound control loop must not meet the driver's allocation lock on its hot path; a
+ * plug-in may simply be handed its input and output buffers and forbidden everything else.  This
+ * entry point calls no cudaMalloc / cudaMallocAsync / cudaFree and no allocating library
+ * routine, ever: the descriptors live in a fixed 1 MiB `static __device__` array inside the
+ * library image.  Every GPU on which the library's code is loaded holds that 1 MiB until the
+ * process exits, used or not.
+ *
+ * Limit.  65 535 tiles.  A tile is 4096 elements (fp32) or 8192 elements (bf16) when a, u, h are
+ * 16-byte aligned and L is a multiple of 4 (fp32) / 8 (bf16); otherwise the scalar-access
+ * kernel runs with 1024-element tiles.  So num_seq*L may be at most 268 431 360 (fp32),
+ * 536 862 720 (bf16) or 67 107 840 (scalar fallback):
+ * affine_scan_static_scratch_max_elements(io_dtype, vectorised) returns these.  Anything larger
+ * returns AFFINESCAN_ERR_TOO_LARGE before any device work; use affine_scan for it.
+ *
+ * Sharing.  There is ONE array per GPU and every call on that GPU uses it.  It keeps what the
+ * previous call wrote; each call zeroes the two counters that must start at zero (an 8-byte
+ * cudaMemsetAsync on `cuda_stream`) and relies on the per-launch epoch in the descriptors for the
+ * rest.  Calls that can overlap on the GPU — two streams, two host threads, a second process
+ * does NOT count (it has its own copy) — RACE on the array and give wrong results or hang:
+ * keep all calls on one stream, or order them with events.
+ *
+ * First call.  The first call on each device looks up the array's device address
+ * (cudaGetSymbolAddress, which may make the driver load the library's code onto that device).
+ * Make that first call outside any stream capture, with the device current that the later calls
+ * will use.
+ *
+ * Asynchronous on cuda_stream like affine_scan; num_seq == 0 or L == 0 is OK.
+ * ------------------------------------------------------------------------------------ */
+AFFINESCAN_API int affine_scan_static_scratch(const void* a, const void* u, const float* h0,
+                                              void* h, float* h_last, int64_t num_seq, int64_t L,
+                                              int io_dtype, void* cuda_stream);
+/* Largest num_seq*L affine_scan_static_scratch accepts for io_dtype on its vector path
+ * (vectorised != 0) or its scalar-access fallback (vectorised == 0); 0 for an unknown dtype.
+ * No device work. */
+AFFINESCAN_API int64_t affine_scan_static_scratch_max_elements(int io_dtype, int vectorised);
 
 /* ------------------------------------------------------------------------------------
  * selective_scan_fwd — Mamba-style fused forward selective scan (BJ north_star):

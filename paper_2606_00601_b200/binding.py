@@ -47,6 +47,8 @@ _SIGNATURES = {
     "affine_scan": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _vp]),
     "affine_scan_ex": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _int, _vp]),
     "affine_scan_host": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _vp]),
+    "affine_scan_static_scratch": (_int, [_vp, _vp, _vp, _vp, _vp, _i64, _i64, _int, _vp]),
+    "affine_scan_static_scratch_max_elements": (_i64, [_int, _int]),
     "selective_scan_fwd": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _vp]),
     "selective_scan_fwd_ex": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _int, _vp]),
     "selective_scan_fwd_host": (_int, [_vp] * 9 + [_int, _int, _int, _i64, _int, _vp]),
@@ -180,6 +182,30 @@ def affine_scan_ex(a, u, h0, h, h_last, variant, stream=None):
     args = _affine_args(a, u, h0, h, h_last, "cuda")
     with torch.cuda.device(a.device):
         _check("affine_scan_ex", load().affine_scan_ex(*args, int(variant), _stream_ptr(stream, a)))
+
+
+def affine_scan_static_scratch(a, u, h0, h, h_last, stream=None):
+    """affine_scan for callers that may not allocate device memory (a server that gave all of
+    HBM to its own cache, an allocator that must own every byte, a loop that cannot afford the
+    driver's allocation lock): the look-back descriptors sit in a fixed 1 MiB array inside the
+    library instead of cudaMallocAsync scratch.  Same result as
+    ``affine_scan_ex(..., AFFINE_LOOKBACK)``.  Raises ``AffineScanError`` with status 6 when
+    ``num_seq * L`` exceeds ``affine_scan_static_scratch_max_elements``.  Every call on a GPU
+    shares that one array: calls that may overlap on the GPU race, so keep them on one stream.
+    Make the first call on each device outside stream capture (it looks up the array's address).
+    """
+    args = _affine_args(a, u, h0, h, h_last, "cuda")
+    with torch.cuda.device(a.device):
+        _check("affine_scan_static_scratch",
+               load().affine_scan_static_scratch(*args, _stream_ptr(stream, a)))
+
+
+def affine_scan_static_scratch_max_elements(io_dtype, vectorised=True) -> int:
+    """Largest ``num_seq * L`` affine_scan_static_scratch accepts (``io_dtype``: a torch dtype or
+    F32 / BF16; ``vectorised=False``: the limit of the scalar-access fallback)."""
+    if isinstance(io_dtype, torch.dtype):
+        io_dtype = {torch.float32: F32, torch.bfloat16: BF16}[io_dtype]
+    return int(load().affine_scan_static_scratch_max_elements(int(io_dtype), int(bool(vectorised))))
 
 
 def affine_scan_host(a, u, h0, h, h_last, stream=None):

@@ -18,7 +18,7 @@ CSRC = os.path.join(PKG_DIR, "csrc")
 LIB_PATH = os.path.join(PKG_DIR, "libaffinescan.so")
 SOURCES = [os.path.join(CSRC, n) for n in
            ("affinescan_api.cu", "affinescan_affine.cu", "affinescan_selective.cu",
-            "affinescan_bwd.cu")]
+            "affinescan_bwd.cu", "affinescan_static_scratch.cu")]
 NVCC_COMPILE_FLAGS = [
     "-std=c++17", "-O3", "-lineinfo",
     "-gencode", "arch=compute_100a,code=sm_100a",

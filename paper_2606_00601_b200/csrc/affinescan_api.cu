@@ -548,6 +548,9 @@ const char* affinescan_status_string(int status)
     case AFFINESCAN_ERR_DTYPE: return "unknown io dtype";
     case AFFINESCAN_ERR_UNSUPPORTED: return "unsupported N, variant, option or shape for the forced variant";
     case AFFINESCAN_ERR_CUDA: return "CUDA runtime error (see affinescan_last_cuda_error)";
+    case AFFINESCAN_ERR_TOO_LARGE:
+        return "problem exceeds the fixed scratch of affine_scan_static_scratch (65535 tiles); "
+               "use affine_scan";
     default: return "unknown status";
     }
 }

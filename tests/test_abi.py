@@ -16,6 +16,7 @@ EXPECTED = {
     "affinescan_status_string", "affinescan_last_cuda_error", "affinescan_last_variant",
     "affinescan_launch_count", "affinescan_version", "affinescan_release_cache",
     "affinescan_set_option",
+    "affine_scan_static_scratch", "affine_scan_static_scratch_max_elements",
 }
 
 
@@ -43,8 +44,8 @@ def test_header_cites_the_paper_for_each_operation():
 
 def test_status_strings():
     assert lib.status_string(0) == "ok"
-    seen = {lib.status_string(i) for i in range(6)}
-    assert len(seen) == 6
+    seen = {lib.status_string(i) for i in range(7)}
+    assert len(seen) == 7
     assert lib.status_string(99) == "unknown status"
 
 

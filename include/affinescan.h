@@ -21,7 +21,13 @@
  *     look-back tile descriptors.  It is allocated, grown and cleared IN STREAM ORDER on
  *     `cuda_stream` (cudaMallocAsync / cudaFreeAsync / cudaMemsetAsync): no device entry
  *     point synchronises the host or the device, and none clears the scratch per call
- *     (descriptor statuses carry a per-launch epoch).  Device entry points may be captured
+ *     (descriptor statuses carry a per-launch epoch).  At most 64 such buffers are kept per
+ *     device (least recently used freed first, in stream order), keyed by the stream's id, so
+ *     buffers of destroyed streams neither pile up nor get inherited by a stream that reuses
+ *     the handle.  The large workspace of selective_scan_bwd is NOT cached: it is a per-call
+ *     cudaMallocAsync / cudaFreeAsync on `cuda_stream` (memory goes back to the device's
+ *     stream-ordered pool, where the caller's allocator policy decides what happens to it).
+ *     affine_scan_static_scratch allocates nothing at all.  Device entry points may be captured
  *     in a CUDA graph: inside a capture the scratch is a per-call stream-ordered
  *     allocation owned by the graph.  A captured graph must not run concurrently with
  *     itself.  Calls on different streams may run concurrently from different threads.
@@ -61,7 +67,8 @@ typedef enum affinescan_status {
     AFFINESCAN_ERR_CUDA = 5,        /* a CUDA runtime call failed; see
                                        affinescan_last_cuda_error()                       */
     AFFINESCAN_ERR_TOO_LARGE = 6    /* the problem needs more scratch than the fixed array of
-                                       affine_scan_static_scratch holds                   */
+                                       affine_scan_static_scratch, or the workspace given
+                                       to selective_scan_bwd_ws, holds                    */
 } affinescan_status;
 
 typedef enum affinescan_dtype {
@@ -266,8 +273,10 @@ AFFINESCAN_API int selective_scan_fwd_host(const void* x, const void* delta, con
  *   reset       [batch, L]           uint8      in, NULL => no resets
  *   a_structure an affinescan_a_structure the caller asserts about A (0 = general)
  *   variant     AFFINESCAN_VARIANT_AUTO or an AFFINESCAN_SELECTIVE_*
- * softplus is evaluated as log2(1 + 2^(v log2 e)) ln 2 with MUFU.EX2 / MUFU.LG2 (v > 20: v;
- * small 2^..: its series), silu with MUFU.EX2 / MUFU.RCP.
+ * softplus(v) is evaluated as max(v, 0) + log1p(e) with e = 2^(-|v| log2 e) in (0, 1] (MUFU.EX2):
+ * log1p(e) = log2(1 + e) ln 2 (MUFU.LG2) for e >= 0.01 and the series e - e^2/2 + e^3/3 below
+ * that, so it is finite for every v and a tiny Delta keeps its relative accuracy; silu with
+ * MUFU.EX2 / MUFU.RCP (fp32 io) or one MUFU.TANH (bf16 io).
  * ------------------------------------------------------------------------------------ */
 AFFINESCAN_API int selective_scan_fwd_ext(const void* x, const void* delta, const float* A,
                                           const void* B, const void* C, const float* D,
@@ -347,9 +356,12 @@ AFFINESCAN_API int affinescan_compose_carry(const float* P_all, const float* U_a
  *   dh0          [batch, d_inner, N] fp32      out
  * Every output pointer may be NULL (=> not written).  All gradients are fp32 whatever the io
  * dtype; sums over rows and batches are formed in a fixed order (bitwise reproducible).
- * Supported shapes: N == 16, d_inner % 32 == 0, L % 8 == 0, 16-byte aligned pointers (dx and
- * ddelta included); anything
- * else returns AFFINESCAN_ERR_UNSUPPORTED.  Asynchronous on cuda_stream.
+ * Supported shapes: N == 16, d_inner % 32 == 0, L % 8 == 0, batch <= 65535, 16-byte aligned
+ * pointers (dx and ddelta included); anything else returns AFFINESCAN_ERR_UNSUPPORTED before any
+ * device work.  This is the backward of the PLAIN forward only: selective_scan_fwd_ext /
+ * _gated (softplus/bias prologue, silu(z) gate, resets) have no backward here — differentiate
+ * those steps outside (dz, dbias and the softplus factor on ddelta are elementwise).
+ * Asynchronous on cuda_stream.
  * ------------------------------------------------------------------------------------ */
 AFFINESCAN_API int selective_scan_bwd(const void* x, const void* delta, const float* A,
                                       const void* B, const void* C, const float* D,
@@ -357,6 +369,25 @@ AFFINESCAN_API int selective_scan_bwd(const void* x, const void* delta, const fl
                                       float* dx, float* ddelta, float* dA, float* dB, float* dC,
                                       float* dD, float* dh0, int batch, int d_inner, int N,
                                       int64_t L, int io_dtype, void* cuda_stream);
+
+/* Same with a CALLER-PROVIDED workspace, so that the caller's own allocator owns (and can cache,
+ * account for and reclaim) the ~16 bytes per (b,d,t) the backward pass needs: `workspace` is a
+ * device buffer of at least selective_scan_bwd_workspace_bytes(batch, d_inner, N, L) bytes,
+ * 16-byte aligned, used from the call until its kernels finish on cuda_stream; contents on
+ * entry do not matter and are garbage afterwards.  workspace == NULL => selective_scan_bwd
+ * (per-call cudaMallocAsync).  A buffer that is too small or misaligned returns
+ * AFFINESCAN_ERR_TOO_LARGE before any device work.  With a workspace the call allocates
+ * nothing. */
+AFFINESCAN_API int selective_scan_bwd_ws(const void* x, const void* delta, const float* A,
+                                         const void* B, const void* C, const float* D,
+                                         const float* h0, const void* dy, const float* dh_last,
+                                         float* dx, float* ddelta, float* dA, float* dB, float* dC,
+                                         float* dD, float* dh0, int batch, int d_inner, int N,
+                                         int64_t L, int io_dtype, void* workspace,
+                                         int64_t workspace_bytes, void* cuda_stream);
+/* Bytes of workspace selective_scan_bwd needs for this shape; 0 for an empty or unsupported
+ * shape.  No device work. */
+AFFINESCAN_API int64_t selective_scan_bwd_workspace_bytes(int batch, int d_inner, int N, int64_t L);
 
 /* ------------------------------------------------------------------------------------
  * Introspection (no device work)
@@ -370,6 +401,9 @@ AFFINESCAN_API int affinescan_last_cuda_error(void);
 AFFINESCAN_API int affinescan_last_variant(void);
 /* Number of kernel launches this process has issued through the library so far. */
 AFFINESCAN_API int64_t affinescan_launch_count(void);
+/* Number of look-back scratch buffers the library currently caches on the current device
+ * (never more than 64; see the conventions at the top). */
+AFFINESCAN_API int affinescan_cached_scratch_buffers(void);
 /* Library version: major*10000 + minor*100 + patch. */
 AFFINESCAN_API int affinescan_version(void);
 /* Tuning knobs for ablations and sweeps (process-wide; -1 restores the default chosen from

@@ -59,11 +59,14 @@ _SIGNATURES = {
     "selective_scan_slice_aggregate": (_int, [_vp] * 7 + [_int, _int, _int, _i64, _int, _vp]),
     "affinescan_compose_carry": (_int, [_vp] * 4 + [_int, _int, _i64, _vp]),
     "selective_scan_bwd": (_int, [_vp] * 16 + [_int, _int, _int, _i64, _int, _vp]),
+    "selective_scan_bwd_ws": (_int, [_vp] * 16 + [_int, _int, _int, _i64, _int, _vp, _i64, _vp]),
+    "selective_scan_bwd_workspace_bytes": (_i64, [_int, _int, _int, _i64]),
     "affinescan_status_string": (ctypes.c_char_p, [_int]),
     "affinescan_last_cuda_error": (_int, []),
     "affinescan_last_variant": (_int, []),
     "affinescan_launch_count": (_i64, []),
     "affinescan_version": (_int, []),
+    "affinescan_cached_scratch_buffers": (_int, []),
     "affinescan_release_cache": (_int, []),
     "affinescan_set_option": (_int, [_int, _int]),
 }
@@ -299,9 +302,18 @@ def selective_scan_fwd_gated(x, delta_raw, delta_bias, A, B, C, D, z, h0, y, h_l
                                                batch, d_inner, N, L, io, _stream_ptr(stream, x)))
 
 
+def selective_scan_bwd_workspace_bytes(batch, d_inner, N, L) -> int:
+    return int(load().selective_scan_bwd_workspace_bytes(int(batch), int(d_inner), int(N), int(L)))
+
+
 def selective_scan_bwd(x, delta, A, B, C, D, h0, dy, dh_last, dx, ddelta, dA, dB, dC, dD, dh0,
-                       stream=None):
-    """Gradients of <dy, y> + <dh_last, h_last> of selective_scan_fwd; outputs fp32, may be None."""
+                       stream=None, workspace="torch"):
+    """Gradients of <dy, y> + <dh_last, h_last> of selective_scan_fwd; outputs fp32, may be None.
+
+    ``workspace``: "torch" (default) takes the ~16 B per (b,d,t) of scratch from torch's caching
+    allocator for this call, so torch sees, reuses and can reclaim it; a uint8 device tensor of at
+    least ``selective_scan_bwd_workspace_bytes`` is used as is; None lets the library take it
+    from cudaMallocAsync per call (the plain C entry point)."""
     batch, d_inner, L = x.shape
     N = A.shape[1]
     f32 = torch.float32
@@ -325,9 +337,27 @@ def selective_scan_bwd(x, delta, A, B, C, D, h0, dy, dh_last, dx, ddelta, dA, dB
         _ptr(dh0, dtype=f32, shape=bdn, device="cuda", name="dh0"),
     )
     with torch.cuda.device(x.device):
-        _check("selective_scan_bwd",
-               load().selective_scan_bwd(*args, batch, d_inner, N, L, _io_dtype(x),
-                                         _stream_ptr(stream, x)))
+        sp = _stream_ptr(stream, x)
+        if isinstance(workspace, str):
+            if workspace != "torch":
+                raise ValueError("workspace must be 'torch', a uint8 device tensor or None")
+            nbytes = selective_scan_bwd_workspace_bytes(batch, d_inner, N, L)
+            # a raw stream handle cannot be recorded on a torch tensor: the library allocates then
+            torch_stream = stream if isinstance(stream, torch.cuda.Stream) else \
+                (torch.cuda.current_stream(x.device) if stream is None else None)
+            workspace = None
+            if nbytes > 0 and torch_stream is not None:
+                workspace = torch.empty(nbytes, dtype=torch.uint8, device=x.device)
+                workspace.record_stream(torch_stream)
+        if workspace is None:
+            _check("selective_scan_bwd",
+                   load().selective_scan_bwd(*args, batch, d_inner, N, L, _io_dtype(x), sp))
+        else:
+            _check("selective_scan_bwd_ws",
+                   load().selective_scan_bwd_ws(
+                       *args, batch, d_inner, N, L, _io_dtype(x),
+                       _ptr(workspace, dtype=torch.uint8, device="cuda", name="workspace"),
+                       workspace.numel(), sp))
 
 
 def selective_scan_slice_aggregate(x, delta, A, B, C, P, U, stream=None):
@@ -396,6 +426,12 @@ def launch_count() -> int:
 
 def version() -> int:
     return load().affinescan_version()
+
+
+def cached_scratch_buffers(device=None) -> int:
+    """Look-back scratch buffers the library caches on ``device`` (default: current)."""
+    with torch.cuda.device(device):
+        return load().affinescan_cached_scratch_buffers()
 
 
 def release_cache() -> None:

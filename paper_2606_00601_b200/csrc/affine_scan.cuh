@@ -410,7 +410,12 @@ affine_scan_chain_kernel(const T* __restrict__ a, const T* __restrict__ u,
         if (lane == 0) {
             for (unsigned it = 0;; ++it) {
                 const int st = static_cast<int>(it % STAGES);
-                if (it >= STAGES) mbar_wait(&empty[st], ((it / STAGES) - 1u) & 1u);
+                if (it >= STAGES) {
+                    mbar_wait(&empty[st], ((it / STAGES) - 1u) & 1u);
+                    // the consumers read this slot through the generic proxy; order those reads
+                    // before the async-proxy overwrite below
+                    fence_proxy_async_smem();
+                }
                 const long long tk = static_cast<long long>(atomicAdd(&ctrl->ticket, 1u));
                 if (tk >= ntiles) {
                     s_tile[st] = -1;

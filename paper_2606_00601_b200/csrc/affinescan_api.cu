@@ -27,9 +27,12 @@ std::mutex g_mu;  // guards the maps below (never held across a device wait)
 struct Buffer {
     void* ptr = nullptr;
     size_t bytes = 0;
+    cudaEvent_t last_use = nullptr;  // recorded by scratch_release after the last launch
+    uint64_t tick = 0;               // LRU clock
 };
-using ScratchKey = std::tuple<int, void*, int>;  // (device, stream, slot)
+using ScratchKey = std::tuple<int, unsigned long long, int>;  // (device, stream id, slot)
 std::map<ScratchKey, Buffer> g_scratch;
+uint64_t g_scratch_tick = 0;
 
 std::map<int, int> g_sm_count;
 
@@ -85,6 +88,36 @@ int allow_dynamic_smem(const void* kernel, int bytes)
     return AFFINESCAN_OK;
 }
 
+namespace {
+
+// Frees the least recently used cached buffers of `dev` (never `keep`) until at most
+// kScratchMaxEntries remain.  The free is enqueued on the CALLER's stream behind the buffer's
+// last-use event, so it is safe whether or not the buffer's own stream still exists.
+// g_mu is held.
+int scratch_evict_lru(int dev, const ScratchKey& keep, cudaStream_t stream)
+{
+    while (true) {
+        int count = 0;
+        auto victim = g_scratch.end();
+        for (auto it = g_scratch.begin(); it != g_scratch.end(); ++it) {
+            if (std::get<0>(it->first) != dev) continue;
+            ++count;
+            if (it->first == keep) continue;
+            if (victim == g_scratch.end() || it->second.tick < victim->second.tick) victim = it;
+        }
+        if (count <= kScratchMaxEntries || victim == g_scratch.end()) return AFFINESCAN_OK;
+        Buffer b = victim->second;
+        g_scratch.erase(victim);
+        if (b.last_use) {
+            AS_CUDA(cudaStreamWaitEvent(stream, b.last_use, 0));
+            AS_CUDA(cudaEventDestroy(b.last_use));  // released once the wait has completed
+        }
+        if (b.ptr) AS_CUDA(cudaFreeAsync(b.ptr, stream));
+    }
+}
+
+}  // namespace
+
 int scratch_acquire(cudaStream_t stream, int slot, size_t bytes, Scratch* out)
 {
     *out = Scratch{};
@@ -100,8 +133,14 @@ int scratch_acquire(cudaStream_t stream, int slot, size_t bytes, Scratch* out)
     }
     int dev = 0;
     AS_CUDA(cudaGetDevice(&dev));
+    unsigned long long sid = 0;
+    AS_CUDA(cudaStreamGetId(stream, &sid));
+    const ScratchKey key{dev, sid, slot};
     std::lock_guard<std::mutex> lk(g_mu);
-    Buffer& b = g_scratch[ScratchKey{dev, static_cast<void*>(stream), slot}];
+    const bool is_new = g_scratch.find(key) == g_scratch.end();
+    Buffer& b = g_scratch[key];
+    b.tick = ++g_scratch_tick;
+    if (is_new) AS_TRY(scratch_evict_lru(dev, key, stream));
     if (b.bytes < bytes) {
         // grow in stream order: earlier calls on this stream that still use the old buffer
         // finish before the free takes effect; nothing synchronises the host
@@ -115,13 +154,44 @@ int scratch_acquire(cudaStream_t stream, int slot, size_t bytes, Scratch* out)
         out->fresh = true;
     }
     out->ptr = b.ptr;
+    out->device = dev;
+    out->stream_id = sid;
+    out->slot = slot;
+    return AFFINESCAN_OK;
+}
+
+int workspace_acquire(cudaStream_t stream, size_t bytes, Scratch* out)
+{
+    *out = Scratch{};
+    AS_CUDA(cudaMallocAsync(&out->ptr, bytes > 0 ? bytes : 1, stream));
+    out->temporary = true;
+    out->fresh = true;
     return AFFINESCAN_OK;
 }
 
 int scratch_release(cudaStream_t stream, const Scratch& s)
 {
-    if (s.temporary && s.ptr) AS_CUDA(cudaFreeAsync(s.ptr, stream));
+    if (!s.ptr) return AFFINESCAN_OK;
+    if (s.temporary) {
+        AS_CUDA(cudaFreeAsync(s.ptr, stream));
+        return AFFINESCAN_OK;
+    }
+    // cached buffer: remember where its last use ends, for a later eviction from another stream
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_scratch.find(ScratchKey{s.device, s.stream_id, s.slot});
+    if (it == g_scratch.end() || it->second.ptr != s.ptr) return AFFINESCAN_OK;  // already evicted
+    if (!it->second.last_use)
+        AS_CUDA(cudaEventCreateWithFlags(&it->second.last_use, cudaEventDisableTiming));
+    AS_CUDA(cudaEventRecord(it->second.last_use, stream));
     return AFFINESCAN_OK;
+}
+
+int scratch_cached_entries(int device)
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    int n = 0;
+    for (const auto& kv : g_scratch) n += std::get<0>(kv.first) == device;
+    return n;
 }
 
 namespace {
@@ -549,8 +619,8 @@ const char* affinescan_status_string(int status)
     case AFFINESCAN_ERR_UNSUPPORTED: return "unsupported N, variant, option or shape for the forced variant";
     case AFFINESCAN_ERR_CUDA: return "CUDA runtime error (see affinescan_last_cuda_error)";
     case AFFINESCAN_ERR_TOO_LARGE:
-        return "problem exceeds the fixed scratch of affine_scan_static_scratch (65535 tiles); "
-               "use affine_scan";
+        return "problem exceeds the fixed scratch of affine_scan_static_scratch (65535 tiles: use "
+               "affine_scan) or the workspace given to selective_scan_bwd_ws";
     default: return "unknown status";
     }
 }
@@ -558,7 +628,16 @@ const char* affinescan_status_string(int status)
 int affinescan_last_cuda_error(void) { return tl_last_cuda_error; }
 int affinescan_last_variant(void) { return tl_last_variant; }
 int64_t affinescan_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
-int affinescan_version(void) { return 200; }
+int affinescan_version(void) { return 300; }
+int affinescan_cached_scratch_buffers(void)
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return 0;
+    }
+    return scratch_cached_entries(dev);
+}
 
 int affinescan_set_option(int key, int value) { return set_lane_row_option(key, value); }
 
@@ -575,6 +654,7 @@ int affinescan_release_cache(void)
         for (auto it = g_scratch.begin(); it != g_scratch.end();) {
             if (std::get<0>(it->first) == dev) {
                 if (it->second.ptr) cudaFree(it->second.ptr);
+                if (it->second.last_use) cudaEventDestroy(it->second.last_use);
                 it = g_scratch.erase(it);
             } else ++it;
         }

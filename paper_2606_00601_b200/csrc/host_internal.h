@@ -42,19 +42,34 @@ int sm_count(int* out);          // cudaDevAttrMultiProcessorCount of the curren
 int allow_dynamic_smem(const void* kernel, int bytes);
 
 // ---- library-owned device scratch, stream-ordered.
-// Outside stream capture: one cached buffer per (device, stream, slot) that only grows; growing
-// frees the old buffer with cudaFreeAsync and allocates with cudaMallocAsync ON THE CALLER'S
-// STREAM, so no entry point ever synchronises the device.  `fresh` tells the caller that the
-// memory is new (zero-filled here, stream-ordered).
+// scratch_acquire — SMALL scratch (look-back descriptors).  Outside stream capture: one cached
+// buffer per (device, stream id, slot) that only grows; growing frees the old buffer with
+// cudaFreeAsync and allocates with cudaMallocAsync ON THE CALLER'S STREAM, so no entry point
+// ever synchronises the device.  The key is cudaStreamGetId, unique for the life of the process,
+// not the raw handle: a new stream that reuses a destroyed stream's handle value never inherits
+// (and races on) that stream's buffer.  At most kScratchMaxEntries buffers are kept per device:
+// beyond that the least recently used one is freed on the caller's stream, ordered after its
+// last use by an event, so buffers of streams that no longer exist do not pile up.  `fresh`
+// tells the caller that the memory is new (zero-filled here, stream-ordered).
 // Inside stream capture: a per-call cudaMallocAsync, zero-filled, that the caller returns with
 // scratch_release (captured as alloc/free nodes, so the graph owns its scratch).
+// workspace_acquire — LARGE per-call workspace (the backward pass): always a per-call
+// cudaMallocAsync, NOT zero-filled, returned to the pool by scratch_release in stream order, so
+// the library never pins hundreds of MB behind the back of the caller's allocator.
 struct Scratch {
     void* ptr = nullptr;
     bool temporary = false;
     bool fresh = false;
+    int device = 0;
+    unsigned long long stream_id = 0;
+    int slot = 0;
 };
+constexpr int kScratchMaxEntries = 64;
 int scratch_acquire(cudaStream_t stream, int slot, size_t bytes, Scratch* out);
+int workspace_acquire(cudaStream_t stream, size_t bytes, Scratch* out);
+// Call after the last launch that uses the scratch (records the last-use event / frees).
 int scratch_release(cudaStream_t stream, const Scratch& s);
+int scratch_cached_entries(int device);  // introspection for tests
 
 // ---- kernels' entry points behind the C ABI (implemented in the other translation units)
 int affine_scan_impl(const void* a, const void* u, const float* h0, void* h, float* h_last,

@@ -17,6 +17,8 @@ EXPECTED = {
     "affinescan_launch_count", "affinescan_version", "affinescan_release_cache",
     "affinescan_set_option",
     "affine_scan_static_scratch", "affine_scan_static_scratch_max_elements",
+    "affinescan_cached_scratch_buffers",
+    "selective_scan_bwd_ws", "selective_scan_bwd_workspace_bytes",
 }
 
 

@@ -34,7 +34,7 @@ def _inputs(batch, d_inner, L, dtype, dev, seed, with_h0=True, with_D=True):
     return inp
 
 
-def gpu_bwd(inp, with_dh_last=True):
+def gpu_bwd(inp, with_dh_last=True, workspace="torch"):
     x = inp["x"]
     batch, d_inner, L = x.shape
     dev = x.device
@@ -45,7 +45,8 @@ def gpu_bwd(inp, with_dh_last=True):
            "dh0": torch.full((batch, d_inner, 16), nan, device=dev)}
     lib.selective_scan_bwd(x, inp["delta"], inp["A"], inp["B"], inp["C"], inp["D"], inp["h0"],
                            inp["dy"], inp["dh_last"] if with_dh_last else None, out["dx"],
-                           out["ddelta"], out["dA"], out["dB"], out["dC"], out["dD"], out["dh0"])
+                           out["ddelta"], out["dA"], out["dB"], out["dC"], out["dD"], out["dh0"],
+                           workspace=workspace)
     torch.cuda.synchronize()
     return out
 
@@ -133,3 +134,26 @@ def test_backward_optional_outputs_empty_and_unsupported(cuda_device):
     bad = _inputs(1, 32, 60, torch.float32, dev, 12)
     with pytest.raises(lib.AffineScanError):
         gpu_bwd(bad)
+
+
+def test_backward_workspace_from_the_caller_from_torch_or_from_the_library(cuda_device):
+    """The ~16 B per (b,d,t) of scratch may come from (i) torch's allocator through the binding
+    (default), (ii) a buffer the caller passes to selective_scan_bwd_ws, (iii) a per-call
+    cudaMallocAsync inside the library: the three give bitwise the same gradients, a dirty
+    workspace changes nothing (every word is written before it is read), and a workspace that is
+    too small is refused before any device work."""
+    inp = _inputs(2, 64, 512, torch.bfloat16, cuda_device, 21)
+    need = lib.selective_scan_bwd_workspace_bytes(2, 64, 16, 512)
+    groups = 2 * 64 // 16
+    assert need == 4 * (groups * (512 // 8) * 16 * 16 + groups * 512 * 32 + 2 * 64 * 16 + 2 * 64)
+    assert lib.selective_scan_bwd_workspace_bytes(2, 65, 16, 512) == 0      # unsupported shape
+    ref = gpu_bwd(inp, workspace="torch")
+    check(inp, "bwd workspace=torch")
+    ws = torch.full((need + 64,), 0xFF, dtype=torch.uint8, device=cuda_device)  # NaN bit patterns
+    for mode in (ws, None):
+        out = gpu_bwd(inp, workspace=mode)
+        for k in NAMES:
+            assert torch.equal(out[k], ref[k]), k
+    with pytest.raises(lib.AffineScanError) as ei:
+        gpu_bwd(inp, workspace=ws[:need - 16])
+    assert ei.value.status == 6

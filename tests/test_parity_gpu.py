@@ -601,3 +601,41 @@ def test_release_cache_then_calls_still_work(cuda_device):
     hh2 = torch.empty_like(a).pin_memory()
     lib.affine_scan_host(a, u, inp["h0"].cpu(), hh2, None)
     assert torch.equal(h, h2) and torch.equal(hl, hl2) and torch.equal(hh, hh2)
+
+
+def test_scratch_cache_is_bounded_keyed_by_stream_id_and_skips_the_backward(cuda_device):
+    """The look-back descriptors are cached per (device, stream id): (i) 80 short-lived streams,
+    each destroyed after its call, leave at most 64 cached buffers (least recently used freed in
+    stream order) and every result stays right, including the streams that inherit a recycled
+    handle; (ii) selective_scan_bwd takes its large workspace per call and caches nothing."""
+    lib.release_cache()
+    assert lib.cached_scratch_buffers() == 0
+    inp = _affine_inputs(2, 50000, torch.float32, cuda_device, 77)
+    href, hlref = oracle_affine(inp)
+    outs = []
+    for i in range(80):
+        s = torch.cuda.Stream(device=cuda_device)
+        s.wait_stream(torch.cuda.current_stream())
+        h = torch.full_like(inp["a"], float("nan"))
+        hl = torch.full((2,), float("nan"), device=cuda_device)
+        lib.affine_scan_ex(inp["a"], inp["u"], inp["h0"], h, hl, lib.AFFINE_LOOKBACK, stream=s)
+        outs.append((h, hl))
+        del s                                   # handle goes back to the driver while work may run
+    torch.cuda.synchronize()
+    n = lib.cached_scratch_buffers()
+    assert 1 <= n <= 64, n
+    for (h, hl) in outs[::7] + outs[-3:]:
+        assert_close(h, href, torch.float32, "many streams h")
+        assert_close(hl, hlref, torch.float32, "many streams h_last")
+    # (ii) the backward pass leaves the cache as it found it
+    c = config(2, batch=1, d_inner=64, N=16, L=256, dtype=torch.float32, seed=5)
+    sel = make_selective_inputs(c, device=cuda_device)
+    dy = torch.ones_like(sel["x"])
+    dx = torch.empty_like(sel["x"])
+    lib.selective_scan_bwd(sel["x"], sel["delta"], sel["A"], sel["B"], sel["C"], sel["D"], None, dy,
+                           None, dx, None, None, None, None, None, None, workspace=None)
+    torch.cuda.synchronize()
+    assert lib.cached_scratch_buffers() == n
+    assert bool(torch.isfinite(dx).all())
+    lib.release_cache()
+    assert lib.cached_scratch_buffers() == 0

@@ -324,7 +324,10 @@ AFFINESCAN_API int affinescan_reset_mask_from_cu_seqlens(const int32_t* cu_seqle
  *   3. affinescan_compose_carry: h_in = (P_{r-1},U_{r-1}) (+) ... (+) (P_0,U_0) applied to h0
  *      (Eq.7);
  *   4. selective_scan_fwd on the slice with h0 = h_in (rank 0 can skip 1-3 and use h0).
- * paper_2606_00601_b200/sharding.py drives the four steps over torch.distributed.
+ * paper_2606_00601_b200/sharding.py drives the four steps over torch.distributed (rank 0 skips
+ * 3, the last rank skips 1).  `delta` here is the step size that enters the recurrence: the
+ * softplus/bias prologue, gate and resets of selective_scan_fwd_ext are NOT part of the slice
+ * aggregate, so apply them before sharding or do not shard the extended forward.
  *
  *   P, U      [batch, d_inner, N] fp32  out          (selective_scan_slice_aggregate)
  *   P_all, U_all [world, n] fp32 in; h0 [n] fp32 in or NULL; h_in [n] fp32 out; n = rows*N

@@ -57,7 +57,17 @@ def selective_scan_fwd_l_sharded(x, delta, A, B, C, D, h0, y, h_last, group=None
         2. all_gather over the ranks                                       [NCCL]
         3. h_in = (P_{r-1},U_{r-1}) (+) ... (+) (P_0,U_0) applied to h0    [kernel]
         4. selective_scan_fwd(slice, h0 = h_in) -> y slice, state after the slice
+    Rank 0 needs no carry (its h_in is h0) and nobody consumes the last rank's aggregate, so rank 0
+    skips step 3 and the last rank skips step 1 (it contributes zeros to the all-gather): with R
+    ranks the extra scan costs R-1 of R slices, and a single rank runs the plain forward only.
     The last rank's state is the global h_last; it is broadcast so every rank returns it.
+
+    ``delta`` is the step size that enters the recurrence, i.e. AFTER any softplus / bias: the
+    prologue, gate and resets of selective_scan_fwd_ext are not threaded through the slice
+    aggregate, so the extended forward cannot be L-sharded with this driver.
+    Unmeasured on more than one GPU: parity is proven with ranks emulated on one B200 and with
+    gloo on CPU; no NCCL timing exists.
+
     ``ops`` injects the three compute steps (tests on CPU pass the oracle); by default they are
     the library's CUDA entry points.  Only plumbing happens here.
     """
@@ -68,18 +78,18 @@ def selective_scan_fwd_l_sharded(x, delta, A, B, C, D, h0, y, h_last, group=None
     batch, d_inner, _ = x.shape
     N = A.shape[1]
     f32 = dict(dtype=torch.float32, device=x.device)
-    P = torch.empty((batch, d_inner, N), **f32)
-    U = torch.empty((batch, d_inner, N), **f32)
-    ops.selective_scan_slice_aggregate(x, delta, A, B, C, P, U)
-    PU = torch.stack([P, U])                                  # one message per rank
+    h_in = h0
     if world > 1:
+        PU = torch.zeros((2, batch, d_inner, N), **f32)       # one message per rank
+        if rank < world - 1:
+            ops.selective_scan_slice_aggregate(x, delta, A, B, C, PU[0], PU[1])
         gathered = [torch.empty_like(PU) for _ in range(world)]
         dist.all_gather(gathered, PU, group=group)
-        PU_all = torch.stack(gathered)                        # [world, 2, batch, d_inner, N]
-    else:
-        PU_all = PU[None]
-    h_in = torch.empty((batch, d_inner, N), **f32)
-    ops.compose_carry(PU_all[:, 0].contiguous(), PU_all[:, 1].contiguous(), h0, h_in, rank)
+        if rank > 0:
+            # ranks 0..rank (the fold reads ranks < rank only; the C call wants rank < rows)
+            PU_all = torch.stack(gathered[:rank + 1])         # [rank+1, 2, batch, d_inner, N]
+            h_in = torch.empty((batch, d_inner, N), **f32)
+            ops.compose_carry(PU_all[:, 0].contiguous(), PU_all[:, 1].contiguous(), h0, h_in, rank)
     state = torch.empty((batch, d_inner, N), **f32)
     ops.selective_scan_fwd(x, delta, A, B, C, D, h_in, y, state)
     if world > 1:

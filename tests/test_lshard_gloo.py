@@ -28,6 +28,8 @@ class OracleOps:
     """The three compute steps of the L-sharded scan, stated with the oracle (float64 inside,
     fp32 tensors at the interface like the CUDA entry points)."""
 
+    calls = {"aggregate": 0, "compose": 0, "fwd": 0}
+
     @staticmethod
     def _np(t):
         return None if t is None else t.double().numpy()
@@ -35,6 +37,7 @@ class OracleOps:
     @classmethod
     def selective_scan_slice_aggregate(cls, x, delta, A, B, C, P, U):
         import oracle
+        cls.calls["aggregate"] += 1
         f = cls._np
         # U: state after the slice entered with h = 0; P: the same call's response to h0 = 1
         # with u = 0 (x = 0): the total product of a_t -- two oracle calls, no closed form
@@ -44,9 +47,11 @@ class OracleOps:
         P.copy_(torch.from_numpy(p))
         U.copy_(torch.from_numpy(u))
 
-    @staticmethod
-    def compose_carry(P_all, U_all, h0, h_in, rank):
+    @classmethod
+    def compose_carry(cls, P_all, U_all, h0, h_in, rank):
         import oracle
+        cls.calls["compose"] += 1
+        assert P_all.shape[0] > rank
         h = np.zeros(tuple(h_in.shape)) if h0 is None else h0.double().numpy().copy()
         for j in range(rank):                     # earlier ranks first; later on the left
             Pj, Uj = P_all[j].double().numpy(), U_all[j].double().numpy()
@@ -58,6 +63,7 @@ class OracleOps:
     @classmethod
     def selective_scan_fwd(cls, x, delta, A, B, C, D, h0, y, h_last):
         import oracle
+        cls.calls["fwd"] += 1
         f = cls._np
         yy, hl = oracle.selective_scan_fwd(f(x), f(delta), f(A), f(B), f(C), f(D), f(h0))
         y.copy_(torch.from_numpy(yy))
@@ -90,6 +96,9 @@ def _worker(rank, world, port, out_dir):
         # the interface tensors of the CUDA path are fp32; the oracle ops accept any float dtype
         selective_scan_fwd_l_sharded(sl["x"], sl["delta"], sl["A"].double(), sl["B"], sl["C"],
                                      sl["D"].double(), sl["h0"].double(), y, h_last, ops=OracleOps)
+        # rank 0 needs no carry, nobody consumes the last rank's aggregate: neither is computed
+        assert OracleOps.calls == {"aggregate": int(rank < world - 1), "compose": int(rank > 0),
+                                   "fwd": 1}, OracleOps.calls
         np.save(os.path.join(out_dir, f"y{rank}.npy"), y.numpy())
         np.save(os.path.join(out_dir, f"hl{rank}.npy"), h_last.numpy())
         dist.barrier()

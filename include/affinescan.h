@@ -41,6 +41,8 @@
  *     AFFINESCAN_SELECTIVE_CHUNKED, whose decoupled look-back folds whichever predecessor
  *     aggregates are published at poll time: reproducible up to the floating-point
  *     association order of P:90 Eq.(7) (all orders are within the stated tolerance).
+ *     AFFINESCAN_VARIANT_AUTO picks these two for one or few long sequences / few rows x long
+ *     L; affinescan_set_option(AFFINESCAN_OPT_DETERMINISTIC, 1) keeps AUTO off them.
  */
 #ifndef AFFINESCAN_H_
 #define AFFINESCAN_H_
@@ -413,9 +415,15 @@ AFFINESCAN_API int affinescan_version(void);
  * the shape).  Returns AFFINESCAN_ERR_UNSUPPORTED for an unknown key or value. */
 typedef enum affinescan_option {
     AFFINESCAN_OPT_LANE_ROW_G = 1,      /* lane_row grid: 1 or 2 lanes per (b,d) row; 3 = balanced mix */
-    AFFINESCAN_OPT_LANE_ROW_POLY16 = 2  /* sixteenths (0 or 4) of the exponentials evaluated by
+    AFFINESCAN_OPT_LANE_ROW_POLY16 = 2, /* sixteenths (0 or 4) of the exponentials evaluated by
                                            the fma-pipe polynomial instead of MUFU.EX2 (one-lane
                                            grid only; the other grids ignore it)                 */
+    AFFINESCAN_OPT_DETERMINISTIC = 3    /* 1: AFFINESCAN_VARIANT_AUTO never picks a decoupled
+                                           look-back schedule (AFFINE_LOOKBACK, SELECTIVE_CHUNKED),
+                                           so every default call is bitwise reproducible run to
+                                           run, at the price of speed on few long sequences / few
+                                           rows; 0 or -1 (default): fastest schedule.  A forced
+                                           variant is never overridden.                          */
 } affinescan_option;
 AFFINESCAN_API int affinescan_set_option(int key, int value);
 /* Frees the cached scratch / staging buffers, copy streams and events of the current device

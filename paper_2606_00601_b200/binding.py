@@ -73,6 +73,7 @@ _SIGNATURES = {
 
 OPT_LANE_ROW_G = 1
 OPT_LANE_ROW_POLY16 = 2
+OPT_DETERMINISTIC = 3
 
 
 class AffineScanError(RuntimeError):

@@ -138,10 +138,17 @@ int affine_dispatch(const void* a_, const void* u_, const float* h0, void* h_, f
             else if (L < 4096)
                 variant = (aligned && !tiny) ? AFFINESCAN_AFFINE_LOOKBACK : AFFINESCAN_AFFINE_CTA_LOOP;
             else
-                variant = (L < (1 << 17) && num_seq >= waves16) ? AFFINESCAN_AFFINE_CTA_LOOP
+                // r03: no upper bound on L here: with >= four waves of sequences the CTA loop
+                // beats the look-back stream at L = 2^17 / 2^18 too (2^30 elements: 1.89 / 1.93
+                // against 2.09 / 2.15 ms)
+                variant = num_seq >= waves16 ? AFFINESCAN_AFFINE_CTA_LOOP
                           : L <= kAffCtaLoopMinL                ? AFFINESCAN_AFFINE_CTA_LOOP
                                                                 : AFFINESCAN_AFFINE_LOOKBACK;
         }
+        // AFFINESCAN_OPT_DETERMINISTIC: the look-back folds whichever aggregates are published
+        // when it polls; the register-carry schedules have one fixed association order
+        if (variant == AFFINESCAN_AFFINE_LOOKBACK && deterministic_auto())
+            variant = AFFINESCAN_AFFINE_CTA_LOOP;
     }
     int st;
     switch (variant) {

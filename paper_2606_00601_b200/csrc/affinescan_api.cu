@@ -20,6 +20,7 @@ namespace {
 thread_local int tl_last_cuda_error = 0;
 thread_local int tl_last_variant = 0;
 std::atomic<int64_t> g_launches{0};
+std::atomic<int> g_opt_deterministic{0};
 
 std::mutex g_mu;  // guards the maps below (never held across a device wait)
 
@@ -53,6 +54,7 @@ int after_launch()
 }
 
 void set_last_variant(int v) { tl_last_variant = v; }
+bool deterministic_auto() { return g_opt_deterministic.load(std::memory_order_relaxed) != 0; }
 
 int sm_count(int* out)
 {
@@ -639,7 +641,15 @@ int affinescan_cached_scratch_buffers(void)
     return scratch_cached_entries(dev);
 }
 
-int affinescan_set_option(int key, int value) { return set_lane_row_option(key, value); }
+int affinescan_set_option(int key, int value)
+{
+    if (key == AFFINESCAN_OPT_DETERMINISTIC) {
+        if (value < -1 || value > 1) return AFFINESCAN_ERR_UNSUPPORTED;
+        g_opt_deterministic.store(value == 1 ? 1 : 0);
+        return AFFINESCAN_OK;
+    }
+    return set_lane_row_option(key, value);
+}
 
 int affinescan_release_cache(void)
 {

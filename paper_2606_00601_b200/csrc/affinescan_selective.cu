@@ -456,7 +456,8 @@ int selective_dispatch(const SelectiveArgs& a, cudaStream_t stream)
                                                            &g_unused)) < 0.85 * c_tma;
         }
         if (lane_ok && lane_wins) variant = AFFINESCAN_SELECTIVE_LANE_ROW;
-        else if (tma_ok && few_rows && t.L >= kChunkedMinL) variant = AFFINESCAN_SELECTIVE_CHUNKED;
+        else if (tma_ok && few_rows && t.L >= kChunkedMinL && !deterministic_auto())
+            variant = AFFINESCAN_SELECTIVE_CHUNKED;
         else if (tma_ok && t.L >= kWarpRowTmaMinL) variant = AFFINESCAN_SELECTIVE_WARP_ROW_TMA;
         else variant = AFFINESCAN_SELECTIVE_WARP_ROW;
     }

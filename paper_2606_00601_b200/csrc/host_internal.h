@@ -105,5 +105,7 @@ int compose_carry_impl(const float* P_all, const float* U_all, const float* h0, 
 int fill_h_last(const float* h0, float* h_last, int64_t n, cudaStream_t stream);
 
 int set_lane_row_option(int key, int value);
+// AFFINESCAN_OPT_DETERMINISTIC: AUTO never picks a decoupled look-back schedule
+bool deterministic_auto();
 
 }  // namespace affinescan_host

@@ -500,9 +500,79 @@ def test_config4_selective_long_sequence_every_element(cuda_device):
     _check_selective_every_element(inp, ref, lib.VARIANT_AUTO, c.dtype, "cfg4 auto")
     auto = lib.last_variant()
     assert auto in FEW_ROWS_VARIANTS
-    for v in SELECTIVE_VARIANTS:
+    # SELECTIVE_CHUNKED too: the decoupled look-back BJ names for this config (plain
+    # instantiation: no bias, gate or resets), 16 fp32 tiles per row
+    for v in SELECTIVE_VARIANTS + [lib.SELECTIVE_CHUNKED]:
         if v != auto:
             _check_selective_every_element(inp, ref, v, c.dtype, f"cfg4 {lib.VARIANT_NAMES[v]}")
+
+
+@pytest.mark.parametrize("dtype", DTYPES)
+def test_selective_chunked_is_what_auto_runs_for_few_rows_and_long_L(cuda_device, dtype):
+    """1 x 128 rows x L = 32 768, no bias / gate / reset: AUTO must send this to the plain
+    instantiation of the chunked look-back schedule, and every element must match the oracle."""
+    inp = _selective_inputs(1, 128, 16, 32768, dtype, cuda_device, seed=4242, with_h0=True)
+    ref = oracle_selective_all_rows(inp, rows_per_task=8)
+    _check_selective_every_element(inp, ref, lib.VARIANT_AUTO, dtype, f"auto few rows {dtype}")
+    assert lib.last_variant() == lib.SELECTIVE_CHUNKED
+
+
+@pytest.mark.parametrize("dtype,L", [(torch.float32, 65536), (torch.bfloat16, 131072)])
+def test_selective_chunked_slow_decay_chain_longer_than_one_lookback_window(cuda_device, dtype, L):
+    """Slow decay (A x 0.05, Delta = softplus(N(-4, 1)) ~ 0.02, h0 given): the product of a over a
+    whole tile stays far from 0 (e^-0.9 .. e^-0.1; the carry over 33 tiles still weighs up to 1.5 %
+    of the state, 150 x the tolerance), so no tile is self-contained and a tile's look-back has to fold
+    AGGREGATE descriptors, and a wrong fold anywhere in the chain shows in the result (with BJ's
+    fast decay a far tile's carry is ~1e-26 of the state and any fold error is invisible).  With
+    ~170 tiles per row, well over the 32 a look-back window covers, the second and later windows
+    run whenever a CTA gets ahead of its predecessors' INCLUSIVE publications.  Three runs: each within the parity bound of the oracle
+    on every element, and within it of each other (the fold order may differ run to run; the
+    header allows exactly that).  (Still slower decay, A x 0.01 with Delta ~ 1e-3, leaves BJ's
+    tolerance in EVERY schedule, this one and the register-carry ones alike: fp32 rounding over a
+    memory of ~1e5 steps.)"""
+    inp = _selective_inputs(1, 64, 16, L, dtype, cuda_device, seed=4343, with_h0=True,
+                            delta_shift=-4.0)
+    inp["A"] = inp["A"] * 0.05
+    ref = oracle_selective_all_rows(inp, rows_per_task=4)
+    # the state really survives the whole sequence: h0's contribution at the end is not negligible
+    assert float(np.abs(ref[1]).max()) > 1e-3
+    outs = []
+    for run in range(3):
+        y, hl = gpu_selective(inp, lib.SELECTIVE_CHUNKED)
+        assert_close_all(y, ref[0], dtype, f"slow decay run {run} y")
+        assert_close_all(hl, ref[1], dtype, f"slow decay run {run} h_last")
+        outs.append((y, hl))
+    for (y, hl) in outs[1:]:
+        assert rel_err(y, outs[0][0].double().cpu().numpy()) <= TOL[dtype]
+        assert rel_err(hl, outs[0][1].double().cpu().numpy()) <= TOL[dtype]
+
+
+def test_deterministic_option_keeps_auto_off_the_lookback_schedules(cuda_device):
+    """affinescan_set_option(AFFINESCAN_OPT_DETERMINISTIC, 1): AUTO takes a register-carry schedule
+    where it would have taken a decoupled look-back, results stay right and are bitwise equal run
+    to run; a forced variant is not overridden; 0 restores the default choice."""
+    ainp = _affine_inputs(1, 1 << 20, torch.float32, cuda_device, 99)
+    sinp = _selective_inputs(1, 128, 16, 32768, torch.float32, cuda_device, seed=98)
+    gpu_affine(ainp)
+    assert lib.last_variant() == lib.AFFINE_LOOKBACK
+    try:
+        lib.set_option(lib.OPT_DETERMINISTIC, 1)
+        h1, hl1 = gpu_affine(ainp)
+        assert lib.last_variant() == lib.AFFINE_CTA_LOOP
+        h2, hl2 = gpu_affine(ainp)
+        assert torch.equal(h1, h2) and torch.equal(hl1, hl2)
+        href, hlref = oracle_affine(ainp)
+        assert_close(h1, href, torch.float32, "deterministic affine")
+        y1, s1 = gpu_selective(sinp)
+        assert lib.last_variant() == lib.SELECTIVE_WARP_ROW_TMA
+        y2, s2 = gpu_selective(sinp)
+        assert torch.equal(y1, y2) and torch.equal(s1, s2)
+        gpu_affine(ainp, lib.AFFINE_LOOKBACK)
+        assert lib.last_variant() == lib.AFFINE_LOOKBACK
+    finally:
+        lib.set_option(lib.OPT_DETERMINISTIC, 0)
+    gpu_selective(sinp)
+    assert lib.last_variant() == lib.SELECTIVE_CHUNKED
 
 
 def test_config5_affine_bandwidth_sweep_every_element(cuda_device):
@@ -529,11 +599,10 @@ def test_config5_affine_bandwidth_sweep_every_element(cuda_device):
         torch.cuda.synchronize()
         if variant == lib.VARIANT_AUTO:
             # fp32 io: up to 2048 steps one single-warp CTA per sequence; longer
-            # ones a CTA each while they are shorter than 2^17 and fill four waves; else the
+            # ones a CTA each while they fill four waves (r03: whatever their length); else the
             # persistent look-back stream
             sms = torch.cuda.get_device_properties(cuda_device).multi_processor_count
-            want = (lib.AFFINE_CTA_LOOP if L <= 2048 or (L < (1 << 17) and S >= 16 * sms)
-                    else lib.AFFINE_LOOKBACK)
+            want = (lib.AFFINE_CTA_LOOP if L <= 2048 or S >= 16 * sms else lib.AFFINE_LOOKBACK)
             assert lib.last_variant() == want
         outs.append((L, S, variant, h, hl))
     h0_host = h0_all.double().cpu().numpy()

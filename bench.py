@@ -495,12 +495,14 @@ def time_backward(cfg, device, local, peak, barrier, K, W):
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
           for _ in range(K)]
     barrier()
+    torch.cuda.profiler.start()      # as in measure(): a profiler sees the timed launches only
     with ClockSampler(local) as clocks:
         for a, b in ev:
             a.record()
             launch()
             b.record()
         torch.cuda.synchronize()
+    torch.cuda.profiler.stop()
     ms = sorted(a.elapsed_time(b) for a, b in ev)
     kernel_ms = sum(ms) / K
     sz = 2 if c.dtype == torch.bfloat16 else 4
@@ -725,6 +727,13 @@ def run_ours(args):
         torch.cuda.empty_cache()
         line["all_configs"] = run_all_configs(args, device, local, peak, sms, barrier,
                                               max_over_ranks)
+        # compact digest LAST in the line (dict order is print order): a log that keeps only the
+        # tail of stdout still shows every config: [workload, kernel, ms, frac of measured HBM,
+        # frac of the MUFU-only wall or null]
+        line["configs_summary"] = [
+            [r["workload"].replace("_selective", "").replace("_affine", ""), r["kernel"],
+             round(r["kernel_ms"], 4), r["hbm_frac"], r.get("frac_of_mufu_only_wall")]
+            for r in line["all_configs"]]
 
     if world > 1:
         import torch.distributed as dist
